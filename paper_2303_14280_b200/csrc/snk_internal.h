@@ -1,0 +1,86 @@
+// snk_internal.h -- host-side context and kernel-launch prototypes of libsnk (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/snk.h"
+
+namespace snk {
+
+constexpr int kTile = 128;          // grid points per CTA of the collocation / integral kernels
+constexpr int kSlotAlign = 32;      // every batch starts on a warp boundary in the slot arrays
+constexpr int kNumClasses = 10;     // (la,lb), la >= lb, la <= 3
+constexpr int kMaxDepth = 20;       // R13
+
+inline int class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }   // (0,0)=0,(1,0)=1,(1,1)=2,(2,0)=3,...
+
+struct PrimPair;   // snk_os.cuh
+
+// One significant shell pair, oriented so that l_a >= l_b (R6); a carries the VRR, the HRR shifts to b.
+struct __align__(16) PairRec {
+  int32_t fa, fb;         // first basis-function index of shell a / b
+  int32_t prim_off;       // first PrimPair
+  int32_t nprim;          // primitive pairs kept (R14)
+  double ABx, ABy, ABz;   // A - B
+  int32_t sa, sb;         // shell ids
+};
+static_assert(sizeof(PairRec) == 48, "PairRec layout");
+
+// One tile = up to kTile consecutive slots of one batch.
+struct TileRec { int32_t batch; int32_t n; int64_t slot; };
+
+// Device shell table (SoA)
+struct ShellTab {
+  const double* cx; const double* cy; const double* cz;
+  const int32_t* l; const int32_t* foff; const int32_t* poff; const int32_t* nprim;
+  const double* pexp; const double* pcoef;
+  const double* rcut2;
+  int nsh; int nbf;
+};
+
+template <class T>
+struct DevBuf {           // grow-only device buffer
+  T* p = nullptr;
+  size_t cap = 0;         // elements
+  cudaError_t reserve(size_t n) {
+    if (n <= cap) return cudaSuccess;
+    if (p) cudaFree(p);
+    p = nullptr; cap = 0;
+    cudaError_t e = cudaMalloc((void**)&p, n * sizeof(T));
+    if (e == cudaSuccess) cap = n;
+    return e;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+  DevBuf() = default;
+  DevBuf(const DevBuf&) = delete;
+  DevBuf& operator=(const DevBuf&) = delete;
+  ~DevBuf() { release(); }
+};
+
+struct IntParams {
+  const double* gx; const double* gy; const double* gz;
+  const double* F; double* G;
+  int64_t ld;              // leading dimension of F/G (slots of the super-batch, padded)
+  int64_t slot0;           // first slot of the super-batch
+  const TileRec* tiles; int ntiles;
+  const uint32_t* vmask; int64_t vstride;   // words per batch
+  int pbeg, pend;          // range of this class in the significant-pair list
+  const PairRec* pairs;
+  const PrimPair* prims;
+  const double* boys;
+};
+
+// ---- kernel launchers (each returns cudaGetLastError()) ----
+cudaError_t launch_integrals(int cls, const IntParams& p, cudaStream_t s);
+cudaError_t launch_debug_A(int la, int lb, bool transpose, const PrimPair* prims, int nprim, double ABx, double ABy, double ABz,
+                           const double* pts, int64_t n, const double* boys, double* out, cudaStream_t s);
+cudaError_t launch_debug_boys(int mmax, int64_t n, const double* x, const double* boys, double* out, cudaStream_t s);
+
+// C[M x N] (beta ? += : =) A[M x K] * op(B);  A row-major lda;  transB=false: B[K x N] row-major ldb;
+// transB=true: B given as [N x K] row-major ldb.  kscale (optional) multiplies A's column k.  fp64 DMMA.
+cudaError_t gemm_f64(bool transB, int64_t M, int64_t N, int64_t K, const double* A, int64_t lda, const double* B, int64_t ldb,
+                     double* C, int64_t ldc, bool beta, const double* kscale, cudaStream_t s);
+
+}  // namespace snk

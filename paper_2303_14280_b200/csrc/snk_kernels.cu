@@ -1,0 +1,607 @@
+// snk_kernels.cu -- everything on the path except the integral kernel and the GEMM:
+//   a0 batching keys / leaves / bboxes (R13)       a1 B_j sphere-box tests (Eq. 41)
+//   Eq. 47 maxima   a3 pair screening (Eqs. 43-46)  a2 collocation (Eq. 31)   a7 symmetrise (Eq. 40)
+#include <cub/cub.cuh>
+
+#include "snk_internal.h"
+#include "snk_kernels.h"
+#include "snk_os.cuh"
+
+namespace snk {
+
+// ------------------------------------------------------------------------------------------------------------
+// a0: keys.  root cell = floor(x/h0) per axis (21 bits each, biased); path = 3 bits per octree level, 20 levels,
+// child bit = (coordinate >= geometric midpoint) -> points on a split plane go to the upper child (R13).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void k_point_keys(int64_t n, const double* __restrict__ pts, const double* __restrict__ w, double h0,
+                             unsigned long long* __restrict__ root, unsigned long long* __restrict__ path, uint32_t* __restrict__ idx,
+                             int* __restrict__ err) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double c[3] = {pts[3 * i], pts[3 * i + 1], pts[3 * i + 2]};
+  const double wi = w[i];
+  if (!(wi >= 0.0) || isinf(wi)) atomicOr(err, 1);
+  unsigned long long r = 0, p = 0;
+  double lo[3], hi[3];
+  bool bad = false;
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    if (!isfinite(c[q])) { bad = true; lo[q] = hi[q] = 0; continue; }
+    const double f = floor(c[q] / h0);
+    if (fabs(f) >= 1048575.0) { bad = true; lo[q] = hi[q] = 0; continue; }
+    const long long ic = (long long)f;
+    r = (r << 21) | (unsigned long long)(ic + 1048576);
+    lo[q] = (double)ic * h0;
+    hi[q] = (double)(ic + 1) * h0;
+  }
+  if (bad) { atomicOr(err, 2); r = 0; }
+  for (int d = 0; d < kMaxDepth; ++d) {
+    unsigned b = 0;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const double mid = 0.5 * (lo[q] + hi[q]);
+      const bool up = c[q] >= mid;
+      b = (b << 1) | (up ? 1u : 0u);
+      if (up) lo[q] = mid; else hi[q] = mid;
+    }
+    p = (p << 3) | b;
+  }
+  root[i] = r; path[i] = p; idx[i] = (uint32_t)i;
+}
+
+template <class T>
+__global__ void k_gather(int64_t n, const uint32_t* __restrict__ idx, const T* __restrict__ src, T* __restrict__ dst) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = src[idx[i]];
+}
+
+// number of points sharing (root, first d levels of path) with sorted position i
+__device__ __forceinline__ int64_t node_count(const unsigned long long* __restrict__ root, const unsigned long long* __restrict__ path,
+                                              int64_t n, int64_t i, int d) {
+  const int sh = 3 * (kMaxDepth - d);
+  const unsigned long long r = root[i], pf = sh >= 60 ? 0ull : (path[i] >> sh);
+  auto less = [&](int64_t k) {      // key(k) < key(i)
+    const unsigned long long rk = root[k];
+    if (rk != r) return rk < r;
+    const unsigned long long pk = sh >= 60 ? 0ull : (path[k] >> sh);
+    return pk < pf;
+  };
+  auto leq = [&](int64_t k) {       // key(k) <= key(i)
+    const unsigned long long rk = root[k];
+    if (rk != r) return rk < r;
+    const unsigned long long pk = sh >= 60 ? 0ull : (path[k] >> sh);
+    return pk <= pf;
+  };
+  int64_t a = 0, b = i;             // first k with !less(k) in [0, i]
+  while (a < b) { const int64_t m = (a + b) >> 1; if (less(m)) a = m + 1; else b = m; }
+  const int64_t first = a;
+  a = i; b = n;                     // first k with !leq(k) in [i, n]
+  while (a < b) { const int64_t m = (a + b) >> 1; if (leq(m)) a = m + 1; else b = m; }
+  return a - first;
+}
+
+// leaf depth of every sorted point: smallest d whose node holds <= nmax points (else kMaxDepth); start flags
+__global__ void k_leaf_depth(int64_t n, const unsigned long long* __restrict__ root, const unsigned long long* __restrict__ path, int nmax,
+                             uint8_t* __restrict__ depth) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int lo = 0, hi = kMaxDepth;       // count is non-increasing in d: find the first d with count <= nmax
+  while (lo < hi) {
+    const int m = (lo + hi) >> 1;
+    if (node_count(root, path, n, i, m) <= nmax) hi = m; else lo = m + 1;
+  }
+  depth[i] = (uint8_t)lo;
+}
+
+__global__ void k_start_flags(int64_t n, const unsigned long long* __restrict__ root, const unsigned long long* __restrict__ path,
+                              const uint8_t* __restrict__ depth, int32_t* __restrict__ flag) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int f = 1;
+  if (i > 0 && root[i] == root[i - 1]) {
+    const int sh = 3 * (kMaxDepth - depth[i]);
+    const unsigned long long a = sh >= 60 ? 0ull : path[i] >> sh, b = sh >= 60 ? 0ull : path[i - 1] >> sh;
+    f = a != b;
+  }
+  flag[i] = f;
+}
+
+// batch_begin[bid] = first sorted position of batch bid (scan = inclusive scan of flags)
+__global__ void k_batch_begin(int64_t n, const int32_t* __restrict__ flag, const int32_t* __restrict__ scan, int64_t* __restrict__ begin) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (flag[i]) begin[scan[i] - 1] = i;
+  if (i == n - 1) begin[scan[i]] = n;
+}
+
+// tight bbox of each batch (exact min/max of its points): one CTA per batch
+__global__ void k_bbox(const int64_t* __restrict__ begin, const uint32_t* __restrict__ idx, const double* __restrict__ pts,
+                       double* __restrict__ bbox) {
+  const int64_t j = blockIdx.x;
+  const int64_t b0 = begin[j], b1 = begin[j + 1];
+  double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int64_t i = b0 + threadIdx.x; i < b1; i += blockDim.x) {
+    const int64_t s = idx[i];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) { const double v = pts[3 * s + q]; lo[q] = fmin(lo[q], v); hi[q] = fmax(hi[q], v); }
+  }
+  __shared__ double slo[3][32], shi[3][32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    for (int o = 16; o; o >>= 1) { lo[q] = fmin(lo[q], __shfl_xor_sync(~0u, lo[q], o)); hi[q] = fmax(hi[q], __shfl_xor_sync(~0u, hi[q], o)); }
+    if (lane == 0) { slo[q][wid] = lo[q]; shi[q][wid] = hi[q]; }
+  }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    const int q = threadIdx.x;
+    double a = slo[q][0], b = shi[q][0];
+    for (int k = 1; k < nw; ++k) { a = fmin(a, slo[q][k]); b = fmax(b, shi[q][k]); }
+    bbox[6 * j + q] = a; bbox[6 * j + 3 + q] = b;
+  }
+}
+
+// a1: shell a in B_j iff dist^2(A, bbox_j) <= rcut_a^2 (R10).  mode 0: count shells per batch; mode 1: bit masks.
+__global__ void k_basis_screen(ShellTab sh, const double* __restrict__ bbox, const int32_t* __restrict__ batch_src, int nbatch, int nshw,
+                               int32_t* __restrict__ count, uint32_t* __restrict__ mask) {
+  const int j = blockIdx.y;
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  const double* bb = bbox + 6 * (int64_t)(batch_src ? batch_src[j] : j);
+  bool in = false;
+  if (a < sh.nsh) {
+    const double c[3] = {sh.cx[a], sh.cy[a], sh.cz[a]};
+    double d2 = 0.0;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const double d = fmax(0.0, fmax(bb[q] - c[q], c[q] - bb[3 + q]));
+      d2 += d * d;
+    }
+    in = d2 <= sh.rcut2[a];
+  }
+  const unsigned bal = __ballot_sync(~0u, in);
+  if ((threadIdx.x & 31) == 0) {
+    if (mask) { if ((a >> 5) < nshw) mask[(int64_t)j * nshw + (a >> 5)] = bal; }
+    else if (bal) atomicAdd(count + j, __popc(bal));
+  }
+}
+
+// slots: batch j occupies [slot, slot + n) (+ padding to kSlotAlign with w = 0 and the batch's first point)
+__global__ void k_fill_slots(const int64_t* __restrict__ bsrc_begin, const int32_t* __restrict__ bn, const int64_t* __restrict__ bslot,
+                             const uint32_t* __restrict__ idx, const double* __restrict__ pts, const double* __restrict__ w,
+                             double* __restrict__ gx, double* __restrict__ gy, double* __restrict__ gz, double* __restrict__ gw,
+                             int64_t* __restrict__ slot_src) {
+  const int j = blockIdx.x;
+  const int64_t b0 = bsrc_begin[j], s0 = bslot[j];
+  const int n = bn[j], npad = (n + kSlotAlign - 1) / kSlotAlign * kSlotAlign;
+  for (int i = threadIdx.x; i < npad; i += blockDim.x) {
+    const int64_t src = idx[b0 + (i < n ? i : 0)];
+    gx[s0 + i] = pts[3 * src]; gy[s0 + i] = pts[3 * src + 1]; gz[s0 + i] = pts[3 * src + 2];
+    gw[s0 + i] = i < n ? w[src] : 0.0;
+    slot_src[s0 + i] = i < n ? src : -1;
+  }
+}
+
+// radial part + components of one shell at displacement (x,y,z); out[ncart(l)]
+__device__ __forceinline__ void shell_eval(const ShellTab& sh, int a, double x, double y, double z, double (&out)[10]) {
+  const double r2 = x * x + y * y + z * z;
+  const int p0 = sh.poff[a], np = sh.nprim[a];
+  double rad = 0.0;
+  for (int k = 0; k < np; ++k) rad = fma(sh.pcoef[p0 + k], exp(-sh.pexp[p0 + k] * r2), rad);
+  switch (sh.l[a]) {
+    case 0: out[0] = rad; break;
+    case 1: out[0] = x * rad; out[1] = y * rad; out[2] = z * rad; break;
+    case 2: {
+      const double xr = x * rad, yr = y * rad;
+      out[0] = x * xr; out[1] = y * xr; out[2] = z * xr; out[3] = y * yr; out[4] = z * yr; out[5] = z * z * rad; break;
+    }
+    default: {
+      const double xx = x * x * rad, yy = y * y * rad, zz = z * z * rad;
+      out[0] = x * xx; out[1] = y * xx; out[2] = z * xx; out[3] = x * yy; out[4] = x * y * z * rad; out[5] = x * zz;
+      out[6] = y * yy; out[7] = z * yy; out[8] = y * zz; out[9] = z * zz; break;
+    }
+  }
+}
+
+// Eq. 47 (R12): PhiTilde_a(j) = max_g max_{mu in a} sqrt(w_g)|Phi[g,mu]| (written per FUNCTION of a),
+//               phitilde(j)  = max_g sqrt(w_g) sum_{mu in B_j} |Phi[g,mu]|.   One CTA per batch.
+constexpr int kMaxPerThread = 16;   // batch_max <= 4096, 256 threads
+__global__ void __launch_bounds__(256) k_maxima(ShellTab sh, const int32_t* __restrict__ bn, const int64_t* __restrict__ bslot,
+                                                const double* __restrict__ gx, const double* __restrict__ gy, const double* __restrict__ gz,
+                                                const double* __restrict__ gw, const uint32_t* __restrict__ bmask, int nshw,
+                                                double* __restrict__ PhiTf, int64_t ldj, double* __restrict__ phit,
+                                                unsigned long long* __restrict__ phimax_bits) {
+  extern __shared__ unsigned long long smax[];     // [nsh] bit patterns of non-negative doubles
+  const int j = blockIdx.x, n = bn[j];
+  const int64_t s0 = bslot[j];
+  for (int a = threadIdx.x; a < sh.nsh; a += blockDim.x) smax[a] = 0ull;
+  __syncthreads();
+  double px[kMaxPerThread], py[kMaxPerThread], pz[kMaxPerThread], sw[kMaxPerThread], sum[kMaxPerThread];
+#pragma unroll
+  for (int q = 0; q < kMaxPerThread; ++q) {
+    const int i = threadIdx.x + q * 256;
+    const bool ok = i < n;
+    px[q] = ok ? gx[s0 + i] : 0.0; py[q] = ok ? gy[s0 + i] : 0.0; pz[q] = ok ? gz[s0 + i] : 0.0;
+    sw[q] = ok ? sqrt(gw[s0 + i]) : -1.0;
+    sum[q] = 0.0;
+  }
+  const uint32_t* m = bmask + (int64_t)j * nshw;
+  for (int wd = 0; wd < nshw; ++wd) {
+    uint32_t bits = m[wd];
+    while (bits) {
+      const int a = (wd << 5) + __ffs(bits) - 1;
+      bits &= bits - 1;
+      const double cx = sh.cx[a], cy = sh.cy[a], cz = sh.cz[a];
+      const int nc = ncart(sh.l[a]);
+      double mx = 0.0;
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) {
+        if (sw[q] < 0.0) continue;
+        double v[10];
+        shell_eval(sh, a, px[q] - cx, py[q] - cy, pz[q] - cz, v);
+        double s = 0.0, vm = 0.0;
+        for (int c = 0; c < nc; ++c) { const double av = fabs(v[c]); s += av; vm = fmax(vm, av); }
+        sum[q] += s;
+        mx = fmax(mx, sw[q] * vm);
+      }
+      for (int o = 16; o; o >>= 1) mx = fmax(mx, __shfl_xor_sync(~0u, mx, o));
+      if ((threadIdx.x & 31) == 0 && mx > 0.0) atomicMax(&smax[a], (unsigned long long)__double_as_longlong(mx));
+    }
+  }
+  double pm = 0.0;
+#pragma unroll
+  for (int q = 0; q < kMaxPerThread; ++q) if (sw[q] >= 0.0) pm = fmax(pm, sw[q] * sum[q]);
+  for (int o = 16; o; o >>= 1) pm = fmax(pm, __shfl_xor_sync(~0u, pm, o));
+  __shared__ unsigned long long spm;
+  if (threadIdx.x == 0) spm = 0ull;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) atomicMax(&spm, (unsigned long long)__double_as_longlong(pm));
+  __syncthreads();
+  if (threadIdx.x == 0) { phit[j] = __longlong_as_double((long long)spm); atomicMax(phimax_bits, spm); }
+  for (int a = threadIdx.x; a < sh.nsh; a += blockDim.x) {
+    const double v = __longlong_as_double((long long)smax[a]);
+    const int f0 = sh.foff[a], nc = ncart(sh.l[a]);
+    for (int c = 0; c < nc; ++c) PhiTf[(int64_t)(f0 + c) * ldj + j] = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3: density-dependent screening
+// ------------------------------------------------------------------------------------------------------------
+__global__ void k_abs(int64_t n, const double* __restrict__ in, double* __restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = fabs(in[i]);
+}
+
+// Ftilde_a(j) = max_{mu in a} Ftf[mu][j]  ->  FtsT[j][a];  Fmax[a] = max_j
+__global__ void k_shell_max(ShellTab sh, int nbatch, const double* __restrict__ Ftf, int64_t ldj, double* __restrict__ FtsT, int nshld,
+                            unsigned long long* __restrict__ Fmax_bits) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int a = blockIdx.y;
+  double v = 0.0;
+  if (j < nbatch) {
+    const int f0 = sh.foff[a], nc = ncart(sh.l[a]);
+    for (int c = 0; c < nc; ++c) v = fmax(v, Ftf[(int64_t)(f0 + c) * ldj + j]);
+    FtsT[(int64_t)j * nshld + a] = v;
+  }
+  for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(~0u, v, o));
+  if ((threadIdx.x & 31) == 0 && v > 0.0) atomicMax(Fmax_bits + a, (unsigned long long)__double_as_longlong(v));
+}
+
+__device__ __forceinline__ bool cand_decode(const PairCand& pc, int64_t i, int& a, int& b) {
+  int c = 0;
+#pragma unroll
+  for (int k = 1; k < kNumClasses; ++k) if (i >= pc.off[k]) c = k;
+  const int64_t r = i - pc.off[c];
+  const int nb = pc.cnt_b[c];
+  const int ia = (int)(r / nb), ib = (int)(r % nb);
+  if (pc.same_l[c] && ia > ib) return false;
+  a = pc.shells[pc.l_off[pc.la[c]] + ia];
+  b = pc.shells[pc.l_off[pc.lb[c]] + ib];
+  return true;
+}
+
+// candidate pair i is globally significant iff its Eq. 44/45 estimate with the per-shell maxima over batches reaches eps
+__global__ void k_pair_flags(PairCand pc, ShellTab sh, const double* __restrict__ Atil, const double* __restrict__ Fmax,
+                             const double* __restrict__ phimax, double eps, int32_t* __restrict__ flag, int32_t* __restrict__ nprim) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= pc.off[kNumClasses]) return;
+  int a, b, f = 0, np = 0;
+  if (cand_decode(pc, i, a, b)) {
+    const double At = Atil[(int64_t)a * sh.nsh + b];
+    const double fa = Fmax[a], fb = Fmax[b];
+    const double eE = fa * fb * At, eK = fmax(fa, fb) * (*phimax) * At;
+    f = (eE >= eps || eK >= eps) ? 1 : 0;
+    np = f ? sh.nprim[a] * sh.nprim[b] : 0;
+  }
+  flag[i] = f; nprim[i] = np;
+}
+
+__global__ void k_pair_compact(PairCand pc, ShellTab sh, const int32_t* __restrict__ flag, const int32_t* __restrict__ pos,
+                               const int32_t* __restrict__ ppos, const double* __restrict__ Atil, PairRec* __restrict__ pairs,
+                               double* __restrict__ pairAt) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= pc.off[kNumClasses] || !flag[i]) return;
+  int a, b;
+  cand_decode(pc, i, a, b);
+  PairRec r;
+  r.fa = sh.foff[a]; r.fb = sh.foff[b]; r.prim_off = ppos[i]; r.nprim = 0;
+  r.ABx = sh.cx[a] - sh.cx[b]; r.ABy = sh.cy[a] - sh.cy[b]; r.ABz = sh.cz[a] - sh.cz[b];
+  r.sa = a; r.sb = b;
+  pairs[pos[i]] = r;
+  pairAt[pos[i]] = Atil[(int64_t)a * sh.nsh + b];
+}
+
+// primitive-pair table of every significant pair (R1 prefactor); R14: a primitive pair whose rigorous s-type bound
+// (same construction as R11) is below prim_thresh / (K_a K_b) is dropped (never when eps = 0).
+__global__ void k_prim_fill(int npair, ShellTab sh, PairRec* __restrict__ pairs, PrimPair* __restrict__ prims, double prim_thresh,
+                            const double* __restrict__ Fmax, const double* __restrict__ phimax) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npair) return;
+  PairRec r = pairs[i];
+  const int a = r.sa, b = r.sb;
+  const int la = sh.l[a], lb = sh.l[b];
+  const int pa = sh.poff[a], pb = sh.poff[b], ka = sh.nprim[a], kb = sh.nprim[b];
+  const double A[3] = {sh.cx[a], sh.cy[a], sh.cz[a]}, B[3] = {sh.cx[b], sh.cy[b], sh.cz[b]};
+  const double AB2 = r.ABx * r.ABx + r.ABy * r.ABy + r.ABz * r.ABz;
+  // density factor of Eqs. 44/45 with the per-shell maxima over batches: the dropped term's effect on K is bounded by bound * dens
+  const double dens = fmax(Fmax[a] * Fmax[b], fmax(Fmax[a], Fmax[b]) * (*phimax));
+  const double thr = prim_thresh / (double)(ka * kb);
+  int n = 0;
+  for (int k = 0; k < ka; ++k)
+    for (int l = 0; l < kb; ++l) {
+      const double za = sh.pexp[pa + k], zb = sh.pexp[pb + l], ca = sh.pcoef[pa + k], cb = sh.pcoef[pb + l];
+      if (prim_thresh > 0.0) {
+        const double zza = la ? 0.5 * za : za, zzb = lb ? 0.5 * zb : zb;
+        const double cca = la ? fabs(ca) * pow((double)la / (2.718281828459045 * za), 0.5 * la) : fabs(ca);
+        const double ccb = lb ? fabs(cb) * pow((double)lb / (2.718281828459045 * zb), 0.5 * lb) : fabs(cb);
+        const double pp = zza + zzb;
+        if (cca * ccb * (6.283185307179586 / pp) * exp(-(zza * zzb / pp) * AB2) * dens < thr) continue;
+      }
+      PrimPair q;
+      q.p = za + zb;
+      q.inv2p = 0.5 / q.p;
+      q.Px = (za * A[0] + zb * B[0]) / q.p; q.Py = (za * A[1] + zb * B[1]) / q.p; q.Pz = (za * A[2] + zb * B[2]) / q.p;
+      q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
+      q.pref = ca * cb * (6.283185307179586 / q.p) * exp(-(za * zb / q.p) * AB2);
+      q.pad = 0.0;
+      prims[r.prim_off + n] = q;
+      ++n;
+    }
+  pairs[i].nprim = n;
+}
+
+// V_j bit masks (Eq. 43): one thread per (batch, significant pair)
+__global__ void k_vmask(int npair, const PairRec* __restrict__ pairs, const double* __restrict__ pairAt, const double* __restrict__ FtsT,
+                        int nshld, const double* __restrict__ phit, double eps, uint32_t* __restrict__ vmask, int64_t vstride) {
+  const int j = blockIdx.y;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool keep = false;
+  if (i < npair) {
+    const double* F = FtsT + (int64_t)j * nshld;
+    const double fa = F[pairs[i].sa], fb = F[pairs[i].sb], At = pairAt[i];
+    const double eE = fa * fb * At, eK = fmax(fa, fb) * phit[j] * At;
+    keep = (eE >= eps || eK >= eps) && pairs[i].nprim > 0;
+  }
+  const unsigned bal = __ballot_sync(~0u, keep);
+  if ((threadIdx.x & 31) == 0 && (i >> 5) < vstride) vmask[(int64_t)j * vstride + (i >> 5)] = bal;
+}
+
+// counters for snk_stats: out[0]=sum|V_j|, [1]=pair-points, [2]=contracted integrals, [3]=primitive integrals,
+// [4..13] contracted integrals per class, [14] flop model
+__global__ void k_vstats(int npair, const PairRec* __restrict__ pairs, ShellTab sh, const int32_t* __restrict__ bn,
+                         const uint32_t* __restrict__ vmask, int64_t vstride, const double* __restrict__ class_flops_prim,
+                         const double* __restrict__ class_flops_contr, double* __restrict__ out) {
+  const int j = blockIdx.y;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npair) return;
+  if (!((vmask[(int64_t)j * vstride + (i >> 5)] >> (i & 31)) & 1u)) return;
+  const PairRec r = pairs[i];
+  const int la = sh.l[r.sa], lb = sh.l[r.sb];
+  const double nq = bn[j], nc = (double)(ncart(la) * ncart(lb));
+  const int cls = la * (la + 1) / 2 + lb;
+  atomicAdd(out + 0, 1.0);
+  atomicAdd(out + 1, nq);
+  atomicAdd(out + 2, nq * nc);
+  atomicAdd(out + 3, nq * nc * r.nprim);
+  atomicAdd(out + 4 + cls, nq * nc);
+  atomicAdd(out + 14, nq * (class_flops_prim[cls] * r.nprim + class_flops_contr[cls]));
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a2: collocation Phi[mu][slot] (Eq. 31), zero for shells outside B_j.  One thread per grid point, one CTA per
+// (tile, chunk of 64 shells); stores are coalesced along the slot index.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kTile) k_colloc(ShellTab sh, const TileRec* __restrict__ tiles, const double* __restrict__ gx,
+                                                  const double* __restrict__ gy, const double* __restrict__ gz,
+                                                  const uint32_t* __restrict__ bmask, int nshw, double* __restrict__ Phi, int64_t ld,
+                                                  int64_t slot0) {
+  const TileRec tile = tiles[blockIdx.x];
+  const int t = threadIdx.x;
+  const int npad = (tile.n + kSlotAlign - 1) / kSlotAlign * kSlotAlign;
+  if (t >= npad) return;
+  const int64_t slot = tile.slot + t;
+  const double x = gx[slot], y = gy[slot], z = gz[slot];
+  double* __restrict__ out = Phi + (slot - slot0);
+  const uint32_t* m = bmask + (int64_t)tile.batch * nshw;
+  const int a0 = blockIdx.y * 64, a1 = min(a0 + 64, sh.nsh);
+  for (int a = a0; a < a1; ++a) {
+    const int f0 = sh.foff[a], nc = ncart(sh.l[a]);
+    if ((m[a >> 5] >> (a & 31)) & 1u) {
+      double v[10];
+      shell_eval(sh, a, x - sh.cx[a], y - sh.cy[a], z - sh.cz[a], v);
+      for (int c = 0; c < nc; ++c) out[(int64_t)(f0 + c) * ld] = v[c];
+    } else {
+      for (int c = 0; c < nc; ++c) out[(int64_t)(f0 + c) * ld] = 0.0;
+    }
+  }
+}
+
+// a7: K = (Kt + Kt^T)/2 (Eq. 40)
+__global__ void k_symmetrise(int n, const double* __restrict__ Kt, double* __restrict__ K) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  for (int r = ty; r < 32; r += 8) {
+    const int i = bx + r, jj = by + tx;            // read Kt[bx-block rows][by-block cols] transposed source
+    tile[r][tx] = (i < n && jj < n) ? Kt[(int64_t)i * n + jj] : 0.0;
+  }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {
+    const int i = by + r, jj = bx + tx;            // K[i][jj] = (Kt[i][jj] + Kt[jj][i])/2 ; Kt[jj][i] = tile[tx][r]
+    if (i < n && jj < n) K[(int64_t)i * n + jj] = 0.5 * (Kt[(int64_t)i * n + jj] + tile[tx][r]);
+  }
+}
+
+__global__ void k_zero_pad_cols(double* __restrict__ A, int64_t rows, int64_t ld, int64_t c0, int64_t c1) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t w = c1 - c0;
+  if (i < rows * w) A[(i / w) * ld + c0 + (i % w)] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host-side launch wrappers
+// ------------------------------------------------------------------------------------------------------------
+static inline unsigned nblk(int64_t n, int b) { return (unsigned)((n + b - 1) / b); }
+
+cudaError_t run_point_keys(int64_t n, const double* pts, const double* w, double h0, unsigned long long* root, unsigned long long* path,
+                           uint32_t* idx, int* err, cudaStream_t s) {
+  if (n > 0) k_point_keys<<<nblk(n, 256), 256, 0, s>>>(n, pts, w, h0, root, path, idx, err);
+  return cudaGetLastError();
+}
+
+cudaError_t run_sort_pairs(void* tmp, size_t& tmp_bytes, const unsigned long long* kin, unsigned long long* kout, const uint32_t* vin,
+                           uint32_t* vout, int64_t n, int end_bit, cudaStream_t s) {
+  return cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, kin, kout, vin, vout, (int)n, 0, end_bit, s);
+}
+
+cudaError_t run_gather_u64(int64_t n, const uint32_t* idx, const unsigned long long* src, unsigned long long* dst, cudaStream_t s) {
+  if (n > 0) k_gather<unsigned long long><<<nblk(n, 256), 256, 0, s>>>(n, idx, src, dst);
+  return cudaGetLastError();
+}
+
+cudaError_t run_leaves(int64_t n, const unsigned long long* root, const unsigned long long* path, int nmax, uint8_t* depth, int32_t* flag,
+                       cudaStream_t s) {
+  if (n > 0) {
+    k_leaf_depth<<<nblk(n, 256), 256, 0, s>>>(n, root, path, nmax, depth);
+    k_start_flags<<<nblk(n, 256), 256, 0, s>>>(n, root, path, depth, flag);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_scan_i32(void* tmp, size_t& tmp_bytes, const int32_t* in, int32_t* out, int64_t n, bool inclusive, cudaStream_t s) {
+  if (inclusive) return cub::DeviceScan::InclusiveSum(tmp, tmp_bytes, in, out, (int)n, s);
+  return cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, in, out, (int)n, s);
+}
+
+cudaError_t run_batch_begin(int64_t n, const int32_t* flag, const int32_t* scan, int64_t* begin, cudaStream_t s) {
+  if (n > 0) k_batch_begin<<<nblk(n, 256), 256, 0, s>>>(n, flag, scan, begin);
+  return cudaGetLastError();
+}
+
+cudaError_t run_bbox(int nbatch, const int64_t* begin, const uint32_t* idx, const double* pts, double* bbox, cudaStream_t s) {
+  if (nbatch > 0) k_bbox<<<nbatch, 256, 0, s>>>(begin, idx, pts, bbox);
+  return cudaGetLastError();
+}
+
+cudaError_t run_basis_screen(const ShellTab& sh, const double* bbox, const int32_t* batch_src, int nbatch, int nshw, int32_t* count,
+                             uint32_t* mask, cudaStream_t s) {
+  if (nbatch > 0) {
+    dim3 g((unsigned)(nshw * 32 + 127) / 128, (unsigned)nbatch);
+    k_basis_screen<<<g, 128, 0, s>>>(sh, bbox, batch_src, nbatch, nshw, count, mask);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_fill_slots(int nbatch, const int64_t* bsrc_begin, const int32_t* bn, const int64_t* bslot, const uint32_t* idx,
+                           const double* pts, const double* w, double* gx, double* gy, double* gz, double* gw, int64_t* slot_src,
+                           cudaStream_t s) {
+  if (nbatch > 0) k_fill_slots<<<nbatch, 256, 0, s>>>(bsrc_begin, bn, bslot, idx, pts, w, gx, gy, gz, gw, slot_src);
+  return cudaGetLastError();
+}
+
+cudaError_t run_maxima(const ShellTab& sh, int nbatch, const int32_t* bn, const int64_t* bslot, const double* gx, const double* gy,
+                       const double* gz, const double* gw, const uint32_t* bmask, int nshw, double* PhiTf, int64_t ldj, double* phit,
+                       unsigned long long* phimax_bits, cudaStream_t s) {
+  if (nbatch > 0) {
+    const size_t sm = (size_t)sh.nsh * sizeof(unsigned long long);
+    if (sm > 48 * 1024) cudaFuncSetAttribute(k_maxima, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_maxima<<<nbatch, 256, sm, s>>>(sh, bn, bslot, gx, gy, gz, gw, bmask, nshw, PhiTf, ldj, phit, phimax_bits);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_abs(int64_t n, const double* in, double* out, cudaStream_t s) {
+  if (n > 0) k_abs<<<nblk(n, 256), 256, 0, s>>>(n, in, out);
+  return cudaGetLastError();
+}
+
+cudaError_t run_shell_max(const ShellTab& sh, int nbatch, const double* Ftf, int64_t ldj, double* FtsT, int nshld,
+                          unsigned long long* Fmax_bits, cudaStream_t s) {
+  if (nbatch > 0) {
+    dim3 g(nblk(nbatch, 128), (unsigned)sh.nsh);
+    k_shell_max<<<g, 128, 0, s>>>(sh, nbatch, Ftf, ldj, FtsT, nshld, Fmax_bits);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_pair_flags(const PairCand& pc, const ShellTab& sh, const double* Atil, const double* Fmax, const double* phimax, double eps,
+                           int32_t* flag, int32_t* nprim, cudaStream_t s) {
+  const int64_t n = pc.off[kNumClasses];
+  if (n > 0) k_pair_flags<<<nblk(n, 256), 256, 0, s>>>(pc, sh, Atil, Fmax, phimax, eps, flag, nprim);
+  return cudaGetLastError();
+}
+
+cudaError_t run_pair_compact(const PairCand& pc, const ShellTab& sh, const int32_t* flag, const int32_t* pos, const int32_t* ppos,
+                             const double* Atil, PairRec* pairs, double* pairAt, cudaStream_t s) {
+  const int64_t n = pc.off[kNumClasses];
+  if (n > 0) k_pair_compact<<<nblk(n, 256), 256, 0, s>>>(pc, sh, flag, pos, ppos, Atil, pairs, pairAt);
+  return cudaGetLastError();
+}
+
+cudaError_t run_prim_fill(int npair, const ShellTab& sh, PairRec* pairs, PrimPair* prims, double prim_thresh, const double* Fmax,
+                          const double* phimax, cudaStream_t s) {
+  if (npair > 0) k_prim_fill<<<nblk(npair, 128), 128, 0, s>>>(npair, sh, pairs, prims, prim_thresh, Fmax, phimax);
+  return cudaGetLastError();
+}
+
+cudaError_t run_vmask(int nbatch, int npair, const PairRec* pairs, const double* pairAt, const double* FtsT, int nshld, const double* phit,
+                      double eps, uint32_t* vmask, int64_t vstride, cudaStream_t s) {
+  if (nbatch > 0 && npair > 0) {
+    dim3 g(nblk(npair, 256), (unsigned)nbatch);
+    k_vmask<<<g, 256, 0, s>>>(npair, pairs, pairAt, FtsT, nshld, phit, eps, vmask, vstride);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_vstats(int nbatch, int npair, const PairRec* pairs, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
+                       int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s) {
+  if (nbatch > 0 && npair > 0) {
+    dim3 g(nblk(npair, 256), (unsigned)nbatch);
+    k_vstats<<<g, 256, 0, s>>>(npair, pairs, sh, bn, vmask, vstride, cfp, cfc, out);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_colloc(const ShellTab& sh, const TileRec* tiles, int ntiles, const double* gx, const double* gy, const double* gz,
+                       const uint32_t* bmask, int nshw, double* Phi, int64_t ld, int64_t slot0, cudaStream_t s) {
+  if (ntiles > 0) {
+    dim3 g((unsigned)ntiles, (unsigned)((sh.nsh + 63) / 64));
+    k_colloc<<<g, kTile, 0, s>>>(sh, tiles, gx, gy, gz, bmask, nshw, Phi, ld, slot0);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_symmetrise(int n, const double* Kt, double* K, cudaStream_t s) {
+  if (n > 0) {
+    dim3 g((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), b(32, 8);
+    k_symmetrise<<<g, b, 0, s>>>(n, Kt, K);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_zero_pad_cols(double* A, int64_t rows, int64_t ld, int64_t c0, int64_t c1, cudaStream_t s) {
+  if (rows > 0 && c1 > c0) k_zero_pad_cols<<<nblk(rows * (c1 - c0), 256), 256, 0, s>>>(A, rows, ld, c0, c1);
+  return cudaGetLastError();
+}
+
+}  // namespace snk

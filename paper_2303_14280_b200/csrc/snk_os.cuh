@@ -1,0 +1,245 @@
+// snk_os.cuh -- device code of the 3c-CP integral kernel: Boys function + Obara-Saika recursions.
+//
+// App. A of arXiv 2303.14280, with the readings R1-R4 of DESIGN.md:
+//   (A3) seed      Theta^n_0 = pref * F_n(p |P - r_g|^2),  pref = c_a c_b (2 pi / p) exp(-mu |A-B|^2)   (R1)
+//   (A1) VRR       Theta^n_{a+1_q} = (P-A)_q Theta^n_a - (P-r_g)_q Theta^{n+1}_a
+//                                    + a_q/(2p) (Theta^n_{a-1_q} - Theta^{n+1}_{a-1_q})                  (R3)
+//   contraction    Theta^0_a summed over primitive pairs between VRR and HRR              (R4)
+//   (A2) HRR       Xi_{a,b+1_q} = Xi_{a+1_q,b} + (A-B)_q Xi_{a,b}, built one b-column at a time and
+//                  merged with the F-contraction so that A is never materialised
+// Everything is compile-time unrolled (templates + constexpr index maps) so the
+// recurrence intermediates live in registers.
+#pragma once
+#include <cuda_runtime.h>
+#include <type_traits>
+
+namespace snk {
+
+__host__ __device__ constexpr int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+// index of component (i,j,k) inside level l=i+j+k; order: i from l down to 0, then j from l-i down to 0
+__host__ __device__ constexpr int cidx(int i, int j, int k) { return (j + k) * (j + k + 1) / 2 + k; }
+// inverse map
+__host__ __device__ constexpr int comp_i(int l, int c) {
+  int ip = 0;
+  while ((ip + 1) * (ip + 2) / 2 <= c) ++ip;
+  return l - ip;
+}
+__host__ __device__ constexpr int comp_k(int l, int c) {
+  int ip = l - comp_i(l, c);
+  return c - ip * (ip + 1) / 2;
+}
+__host__ __device__ constexpr int comp_j(int l, int c) { return l - comp_i(l, c) - comp_k(l, c); }
+// number of components in levels [la, lb]
+__host__ __device__ constexpr int nlev(int la, int lb) {
+  int n = 0;
+  for (int l = la; l <= lb; ++l) n += ncart(l);
+  return n;
+}
+
+template <int B, int E, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (B < E) {
+    f(std::integral_constant<int, B>{});
+    static_for<B + 1, E>(f);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Boys function, Eq. 22, reading R15:
+//   x < xmax(L): 8-term Taylor about the nearest node of a Delta = 1/16 table of F_m(x_i) at the top
+//                order m = L (dF_m/dx = -F_{m+1}), then downward recursion
+//                F_{m-1} = (2x F_m + e^{-x})/(2m-1)
+//   x >= xmax(L): F_0 = sqrt(pi/x)/2 and upward F_{m+1} = (2m+1) F_m / (2x); the neglected e^{-x}
+//                terms are < 4e-16 relative at xmax(L).
+// Table layout: tab[i*kBoysStride + m], m = 0..kBoysOrders-1, built on the host in snk_api.cu.
+// ------------------------------------------------------------------------------------------------
+constexpr int kBoysStride = 16;
+constexpr int kBoysOrders = 14;            // up to L + 7 with L = 6
+constexpr double kBoysDelta = 1.0 / 16.0;
+constexpr int kBoysRows = 52 * 16 + 2;
+__host__ __device__ constexpr double boys_xmax(int L) {
+  return L == 0 ? 34.0 : L == 1 ? 38.0 : L == 2 ? 40.0 : L == 3 ? 44.0 : L == 4 ? 46.0 : L == 5 ? 50.0 : 52.0;
+}
+
+template <int L>
+__device__ __forceinline__ void boys(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
+  if (x < boys_xmax(L)) {
+    const int i = __double2int_rn(x * 16.0);
+    const double d = (double)i * kBoysDelta - x;     // F_m(x) = sum_k F_{m+k}(x_i) d^k / k!
+    const double* row = tab + i * kBoysStride + L;
+    double t[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t[k] = __ldg(row + k);
+    double s = t[7] * (1.0 / 7.0);
+    s = fma(s, d, t[6]) * (1.0 / 6.0);
+    s = fma(s, d, t[5]) * (1.0 / 5.0);
+    s = fma(s, d, t[4]) * (1.0 / 4.0);
+    s = fma(s, d, t[3]) * (1.0 / 3.0);
+    s = fma(s, d, t[2]) * 0.5;
+    s = fma(s, d, t[1]);
+    F[L] = fma(s, d, t[0]);
+    if constexpr (L > 0) {
+      const double ex = exp(-x);
+      const double x2 = 2.0 * x;
+#pragma unroll
+      for (int m = L; m >= 1; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
+    }
+  } else {
+    const double r = rsqrt(x);
+    F[0] = 0.88622692545275801365 * r;               // sqrt(pi)/2
+    if constexpr (L > 0) {
+      const double h = 0.5 * r * r;                  // 1/(2x)
+#pragma unroll
+      for (int m = 0; m < L; ++m) F[m + 1] = (2 * m + 1) * F[m] * h;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// One primitive pair: everything that does not depend on the grid point.
+// ------------------------------------------------------------------------------------------------
+struct __align__(16) PrimPair {
+  double p;        // zeta_a + zeta_b
+  double inv2p;    // 1 / (2p)
+  double Px, Py, Pz;
+  double PAx, PAy, PAz;   // P - A, A = centre of the shell that carries the VRR (first of the pair, l_a >= l_b)
+  double pref;     // c_a c_b (2 pi / p) exp(-zeta_a zeta_b / p |A-B|^2)
+  double pad;
+};
+static_assert(sizeof(PrimPair) == 80, "PrimPair layout");
+
+// offset of level l inside the flat VRR work array: level l holds Theta^n_a, |a| = l, n = 0..L-l, as [n][comp]
+__host__ __device__ constexpr int vrr_off(int L, int l) {
+  int o = 0;
+  for (int m = 0; m < l; ++m) o += ncart(m) * (L - m + 1);
+  return o;
+}
+
+// VRR (A1): acc[] (levels LA..L of Theta^0, contracted, R4) += this primitive pair's values.
+// th0[n] = Theta^n_0 (seed already scaled by pref), n = 0..L.  The work array is flat with compile-time
+// offsets; after unrolling the code is straight-line, so ptxas keeps only live values in registers.
+template <int LA, int L>
+__device__ __forceinline__ void vrr_accumulate(const double (&th0)[L + 1], double PAx, double PAy, double PAz, double PCx,
+                                               double PCy, double PCz, double inv2p, double (&acc)[nlev(LA, L)]) {
+  double v[vrr_off(L, L + 1)];
+#pragma unroll
+  for (int n = 0; n <= L; ++n) v[n] = th0[n];
+  if constexpr (LA == 0) acc[0] += th0[0];
+  static_for<0, L>([&](auto lc) {
+    constexpr int l = decltype(lc)::value;                 // build level l+1 from levels l and l-1
+    constexpr int nc1 = ncart(l + 1), nc0 = ncart(l), ncm = l > 0 ? ncart(l - 1) : 1;
+    constexpr int o1 = vrr_off(L, l + 1), o0 = vrr_off(L, l), om = l > 0 ? vrr_off(L, l - 1) : 0;
+    static_for<0, L - l>([&](auto nn) {
+      constexpr int n = decltype(nn)::value;
+      static_for<0, nc1>([&](auto cc) {
+        constexpr int c = decltype(cc)::value;
+        constexpr int i = comp_i(l + 1, c), j = comp_j(l + 1, c), k = comp_k(l + 1, c);
+        constexpr int q = i > 0 ? 0 : (j > 0 ? 1 : 2);          // lower along the first non-zero direction
+        constexpr int li = i - (q == 0), lj = j - (q == 1), lk = k - (q == 2);
+        constexpr int cl = cidx(li, lj, lk);
+        constexpr int aq = q == 0 ? li : (q == 1 ? lj : lk);     // a_q: quantum before raising
+        const double PAq = q == 0 ? PAx : (q == 1 ? PAy : PAz);
+        const double PCq = q == 0 ? PCx : (q == 1 ? PCy : PCz);
+        double t = fma(PAq, v[o0 + n * nc0 + cl], -PCq * v[o0 + (n + 1) * nc0 + cl]);
+        if constexpr (aq > 0) {
+          constexpr int cll = cidx(li - (q == 0), lj - (q == 1), lk - (q == 2));
+          t = fma((double)aq * inv2p, v[om + n * ncm + cll] - v[om + (n + 1) * ncm + cll], t);
+        }
+        v[o1 + n * nc1 + c] = t;
+        if constexpr (n == 0 && l + 1 >= LA) acc[nlev(LA, l) + c] += t;
+      });
+    });
+  });
+}
+
+// HRR (A2) tree, column by column, merged with the two contractions of Eq. 38 (both directions of the
+// unordered pair, R8):   Ga[i] += A[i,b] Fb[b]     Gb[b] += sum_i A[i,b] Fa[i].
+// W holds (a | b_partial) for a-levels LA..LTOP.
+template <int LA, int LB, int BX, int BY, int BZ, int LTOP>
+struct HrrNode {
+  static constexpr int NA = ncart(LA);
+  template <class Sink>
+  static __device__ __forceinline__ void run(const double (&W)[nlev(LA, LTOP)], double ABx, double ABy, double ABz, Sink& sink) {
+    if constexpr (BX + BY + BZ == LB) {
+      static_assert(LTOP == LA, "HRR bookkeeping");
+      sink.template column<cidx(BX, BY, BZ)>(W);
+    } else {
+      if constexpr (BY == 0 && BZ == 0) shift<0, BX + 1, BY, BZ>(W, ABx, ABx, ABy, ABz, sink);
+      if constexpr (BZ == 0) shift<1, BX, BY + 1, BZ>(W, ABy, ABx, ABy, ABz, sink);
+      shift<2, BX, BY, BZ + 1>(W, ABz, ABx, ABy, ABz, sink);
+    }
+  }
+  template <int Q, int NX, int NY, int NZ, class Sink>
+  static __device__ __forceinline__ void shift(const double (&W)[nlev(LA, LTOP)], double ABq, double ABx, double ABy, double ABz,
+                                               Sink& sink) {
+    double W2[nlev(LA, LTOP - 1)];
+    static_for<LA, LTOP>([&](auto lc) {
+      constexpr int l = decltype(lc)::value;
+      static_for<0, ncart(l)>([&](auto cc) {
+        constexpr int c = decltype(cc)::value;
+        constexpr int i = comp_i(l, c), j = comp_j(l, c), k = comp_k(l, c);
+        constexpr int cu = cidx(i + (Q == 0), j + (Q == 1), k + (Q == 2));    // a + 1_q, level l+1
+        W2[nlev(LA, l - 1) + c] = fma(ABq, W[nlev(LA, l - 1) + c], W[nlev(LA, l) + cu]);
+      });
+    });
+    HrrNode<LA, LB, NX, NY, NZ, LTOP - 1>::run(W2, ABx, ABy, ABz, sink);
+  }
+};
+
+// Sink used by the build: contracts each finished column with F.
+template <int LA, int LB>
+struct ContractSink {
+  static constexpr int NA = ncart(LA), NB = ncart(LB);
+  const double (&Fa)[NA];
+  const double (&Fb)[NB];
+  double (&Ga)[NA];
+  double (&Gb)[NB];
+  template <int CB>
+  __device__ __forceinline__ void column(const double (&col)[NA]) {
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < NA; ++i) {
+      Ga[i] = fma(col[i], Fb[CB], Ga[i]);
+      s = fma(col[i], Fa[i], s);
+    }
+    Gb[CB] += s;
+  }
+};
+
+// Sink used by the test hook: stores the A block.
+template <int LA, int LB>
+struct StoreSink {
+  static constexpr int NA = ncart(LA), NB = ncart(LB);
+  double* out;   // [NA*NB] row-major for this thread
+  template <int CB>
+  __device__ __forceinline__ void column(const double (&col)[NA]) {
+#pragma unroll
+    for (int i = 0; i < NA; ++i) out[i * NB + CB] = col[i];
+  }
+};
+
+// Contracted Theta^0 (levels LA..LA+LB) of one shell pair at one point.
+template <int LA, int LB>
+__device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp, int nprim, double gx, double gy, double gz,
+                                                 const double* __restrict__ boys_tab, double (&acc)[nlev(LA, LA + LB)]) {
+  constexpr int L = LA + LB;
+#pragma unroll
+  for (int i = 0; i < nlev(LA, L); ++i) acc[i] = 0.0;
+  for (int k = 0; k < nprim; ++k) {
+    const double p = __ldg(&pp[k].p);
+    const double PCx = __ldg(&pp[k].Px) - gx, PCy = __ldg(&pp[k].Py) - gy, PCz = __ldg(&pp[k].Pz) - gz;
+    const double x = p * fma(PCx, PCx, fma(PCy, PCy, PCz * PCz));
+    double th0[L + 1];
+    boys<L>(x, boys_tab, th0);
+    const double pref = __ldg(&pp[k].pref);
+#pragma unroll
+    for (int n = 0; n <= L; ++n) th0[n] *= pref;
+    if constexpr (L == 0) {
+      acc[0] += th0[0];
+    } else {
+      vrr_accumulate<LA, L>(th0, __ldg(&pp[k].PAx), __ldg(&pp[k].PAy), __ldg(&pp[k].PAz), PCx, PCy, PCz, __ldg(&pp[k].inv2p), acc);
+    }
+  }
+}
+
+}  // namespace snk

@@ -1,0 +1,198 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded inputs.
+Bar (BASELINE.json north_star): max |dK| <= 1e-10 and relative Frobenius error <= 1e-11, fp64 throughout."""
+import math
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+from paper_2303_14280_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+ABS_TOL = 1e-10
+FRO_TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the product path has no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def snk_mod(torch_cuda):
+    from paper_2303_14280_b200 import snk
+    snk.load()
+    return snk
+
+
+def _check_parity(Kg, Ko, tag=""):
+    d = np.abs(Kg - Ko).max()
+    fro = np.linalg.norm(Kg - Ko) / max(np.linalg.norm(Ko), 1e-300)
+    assert d <= ABS_TOL and fro <= FRO_TOL, "%s: max|dK|=%.3e relF=%.3e (|K|max=%.3e)" % (tag, d, fro, np.abs(Ko).max())
+    return d, fro
+
+
+def test_boys_device_vs_mpmath(snk_mod, torch_cuda):
+    """Eq. 22: device Boys (table + Taylor + downward recursion / asymptotic) vs 40-digit mpmath."""
+    torch = torch_cuda
+    mp.mp.dps = 40
+    xs = [0.0, 1e-12, 1e-6, 1e-3, 0.03, 0.031, 0.0625, 0.1, 0.5, 1.0, 2.7, 7.77, 15.97, 16.0, 16.03125, 25.0, 33.99, 34.0, 34.01, 37.99,
+          38.0, 39.9, 40.0, 43.99, 44.0, 45.99, 46.0, 49.99, 50.0, 51.99, 52.0, 52.01, 60.0, 100.0, 1e3, 1e5]
+    rng = np.random.default_rng(0)
+    xs = np.array(xs + list(rng.uniform(0, 56, 200)))
+    xd = torch.as_tensor(xs, device="cuda")
+    worst = 0.0
+    for mmax in range(7):
+        F = snk_mod.debug_boys(mmax, xd).cpu().numpy()
+        for i, x in enumerate(xs):
+            for m in range(mmax + 1):
+                ref = mp.mpf(1) / (2 * m + 1) if x == 0 else mp.gammainc(m + mp.mpf(1) / 2, 0, mp.mpf(float(x))) / (2 * mp.mpf(float(x)) ** (m + mp.mpf(1) / 2))
+                rel = abs(F[i, m] / float(ref) - 1)
+                worst = max(worst, rel)
+                assert rel <= 1e-14, (mmax, m, x, rel)
+    print("device Boys worst rel err %.2e" % worst)
+
+
+def _stress_basis(seed=11):
+    """two centres carrying s,p,d,f shells with 1-3 primitives: every (la,lb) class incl. same-centre pairs."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    atoms = np.array([[0.0, 0.1, -0.2], [1.1, -0.7, 0.9]])
+    sh = {6: [(0, 3), (1, 2), (2, 1), (3, 2)]}
+    return inputs.make_basis(rng, np.array([6, 6]), atoms, sh, (0.15, 8.0))
+
+
+def test_A_blocks_OS_vs_MD(snk_mod, oracle_mod, torch_cuda):
+    """App. A (Obara-Saika, GPU) vs Eqs. 15-24 (McMurchie-Davidson, oracle): two independent algorithms for Eq. 37."""
+    torch = torch_cuda
+    b = _stress_basis()
+    o = oracle_mod.Oracle(b)
+    s = snk_mod.Snk(b)
+    rng = np.random.default_rng(2)
+    pts = np.concatenate([rng.uniform(-3, 3, (300, 3)), rng.uniform(-40, 40, (100, 3)), b.atom_xyz, b.atom_xyz + 1e-9])
+    pd = torch.as_tensor(pts, device="cuda")
+    worst = 0.0
+    for a in range(b.nshells):
+        for c in range(b.nshells):
+            got = s.debug_A_pair(a, c, pd).cpu().numpy()
+            ref = o.A_pair(a, c, pts)
+            scale = np.abs(ref).max()
+            err = np.abs(got - ref).max() / scale
+            worst = max(worst, err)
+            assert err < 2e-13, (a, c, int(b.shell_l[a]), int(b.shell_l[c]), err)
+    print("A blocks worst rel err %.2e" % worst)
+
+
+def _run_both(snk_mod, oracle_mod, w, *, eps=None, batch_max=2048, batch_cell=6.0, workspace_gb=None, audit=True, tag=""):
+    eps = w.eps if eps is None else eps
+    o = oracle_mod.Oracle(w.basis)
+    o.set_grid(w.points, w.weights, eps=eps, batch_cell=batch_cell, batch_max=batch_max)
+    Ko = o.build_K(w.P)
+    Kg, ctx = snk_mod.build_K(w.basis, w.points, w.weights, w.P, eps=eps, batch_cell=batch_cell, batch_max=batch_max,
+                              workspace_gb=workspace_gb, return_ctx=True)
+    if audit:
+        L = ctx.export_lists()
+        off, perm, _ = o.batches()
+        assert np.array_equal(L["batch_off"], off), tag
+        for j in range(len(off) - 1):          # same batches in the same order (order inside a batch is free)
+            assert set(L["perm"][off[j]:off[j + 1]].tolist()) == set(perm[off[j]:off[j + 1]].tolist()), (tag, j)
+        Boff, Bids = o.B_lists()
+        assert np.array_equal(L["B_off"], Boff) and np.array_equal(L["B_ids"], Bids), tag
+        Voff, Vp = o.V_lists()
+        if not (np.array_equal(L["V_off"], Voff) and np.array_equal(L["V_pairs"], Vp)):
+            bad = [j for j in range(len(Voff) - 1) if (L["V_off"][j + 1] - L["V_off"][j]) != (Voff[j + 1] - Voff[j])]
+            pytest.fail("%s: V_j lists differ oracle vs GPU (batches %s ...)" % (tag, bad[:5]))
+        st = ctx.stats()
+        os_ = o.stats()
+        assert st["n_int_contracted"] == os_["n_int_contracted"], (tag, st["n_int_contracted"], os_["n_int_contracted"])
+    d, fro = _check_parity(Kg, Ko, tag)
+    assert np.array_equal(Kg, Kg.T)
+    print("%s: max|dK|=%.2e relF=%.2e |K|max=%.2e nbatch=%d" % (tag, d, fro, np.abs(Ko).max(), ctx.stats()["nbatch"]))
+    return Kg, Ko, ctx
+
+
+def test_K_cfg1_full(snk_mod, oracle_mod):
+    """BASELINE.json configs[0]: single water, 9 functions, ~7.7k points, no screening."""
+    w = inputs.make_workload(1)
+    _run_both(snk_mod, oracle_mod, w, tag="cfg1")
+
+
+@pytest.mark.parametrize("batch_max,eps", [(2048, 1e-12), (200, 1e-12), (333, 0.0), (2048, 1e-7)])
+def test_K_cfg2_reduced_grid(snk_mod, oracle_mod, batch_max, eps):
+    """8-water config with a reduced grid (oracle finishes in seconds); several batches / tiles / ragged tails."""
+    w = inputs.make_workload(2, grid=(10, 6, 12))
+    _run_both(snk_mod, oracle_mod, w, eps=eps, batch_max=batch_max, tag="cfg2r[%d,%g]" % (batch_max, eps))
+
+
+def test_K_cfg2_superbatches(snk_mod, oracle_mod):
+    """tiny workspace -> several super-batches (Alg. 1 loop)"""
+    w = inputs.make_workload(2, grid=(10, 6, 12))
+    Kg, Ko, ctx = _run_both(snk_mod, oracle_mod, w, batch_max=512, workspace_gb=0.02, tag="cfg2r-super")
+    assert ctx.stats()["nsuper"] > 1
+
+
+def test_K_cfg5_reduced(snk_mod, oracle_mod):
+    """angular-momentum stress (s..f, exponents to 5000): 4 atoms, reduced grid; all ten (la,lb) classes."""
+    w = inputs.make_workload(5, grid=(10, 6, 10), natoms=4)
+    _run_both(snk_mod, oracle_mod, w, tag="cfg5r")
+    _run_both(snk_mod, oracle_mod, w, eps=0.0, batch_max=100, tag="cfg5r-noscreen")
+
+
+def test_K_linearity_and_host_call(snk_mod, oracle_mod, torch_cuda):
+    torch = torch_cuda
+    w = inputs.make_workload(2, grid=(8, 6, 8), lattice=1)
+    s = snk_mod.Snk(w.basis)
+    s.set_option("eps", 0.0)
+    s.set_grid(torch.as_tensor(w.points, device="cuda"), torch.as_tensor(w.weights, device="cuda"))
+    rng = np.random.default_rng(1)
+    C2 = rng.standard_normal((w.basis.nbf, 3))
+    P2 = C2 @ C2.T
+    K1 = s.build_K(torch.as_tensor(w.P, device="cuda")).cpu().numpy()
+    K2 = s.build_K(torch.as_tensor(P2, device="cuda")).cpu().numpy()
+    K12 = s.build_K(torch.as_tensor(0.3 * w.P - 1.1 * P2, device="cuda")).cpu().numpy()
+    assert np.abs(K12 - (0.3 * K1 - 1.1 * K2)).max() < 1e-12 * np.abs(K12).max()
+    Kh = s.build_K_host(np.ascontiguousarray(w.P))
+    assert np.abs(Kh - K1).max() < 1e-13 * np.abs(K1).max()
+
+
+def test_edge_cases(snk_mod, oracle_mod, torch_cuda):
+    torch = torch_cuda
+    w = inputs.make_workload(1, grid=(6, 4, 6))
+    s = snk_mod.Snk(w.basis)
+    P = torch.as_tensor(w.P, device="cuda")
+    # build before grid
+    with pytest.raises(snk_mod.SnkError) as e:
+        s.build_K(P)
+    assert e.value.code == snk_mod.SNK_ESTATE
+    # empty grid -> K = 0
+    s.set_grid(torch.zeros((0, 3), dtype=torch.float64, device="cuda"), torch.zeros(0, dtype=torch.float64, device="cuda"))
+    assert float(s.build_K(P).abs().max()) == 0.0
+    # one point; all-zero weights
+    o = oracle_mod.Oracle(w.basis)
+    for pts, wt in [(w.points[:1], w.weights[:1]), (w.points[:33], w.weights[:33]), (w.points, np.zeros_like(w.weights))]:
+        o.set_grid(pts, wt, eps=0.0)
+        Ko = o.build_K(w.P)
+        s.set_grid(torch.as_tensor(pts, device="cuda"), torch.as_tensor(wt, device="cuda"))
+        _check_parity(s.build_K(P).cpu().numpy(), Ko, "edge n=%d" % len(wt))
+    # negative weight
+    bad = w.weights.copy(); bad[3] = -1.0
+    with pytest.raises(snk_mod.SnkError) as e:
+        s.set_grid(torch.as_tensor(w.points, device="cuda"), torch.as_tensor(bad, device="cuda"))
+    assert e.value.code == snk_mod.SNK_EINVAL
+    # bad basis
+    b = w.basis
+    b2 = inputs.Basis(b.atom_xyz, b.shell_atom, np.full_like(b.shell_l, 4), b.shell_nprim, b.prim_exp, b.prim_coef)
+    with pytest.raises(snk_mod.SnkError) as e:
+        snk_mod.Snk(b2)
+    assert e.value.code == snk_mod.SNK_EINVAL
+    with pytest.raises(snk_mod.SnkError):
+        s.set_option("nonsense", 1.0)
+    # points far outside every cutoff sphere with screening on: every batch dropped -> K = 0
+    s2 = snk_mod.Snk(b)
+    s2.set_option("eps", 1e-10)
+    far = w.points[:100] + 1e4
+    s2.set_grid(torch.as_tensor(far, device="cuda"), torch.as_tensor(w.weights[:100], device="cuda"))
+    assert float(s2.build_K(P).abs().max()) == 0.0
