@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- sn-K build benchmark (BASELINE.json metric: "sn-K build wall-time and integrals/s at 1 B200;
+fraction of FP64 peak").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (rows a2-a7 of DESIGN.md plus the density-dependent screening a3;
+a0/a1 are per-geometry and reported as ``set_grid_ms``) over the synthetic workload: one ``snk_build_K``.
+``value``  = contracted 3c-CP integrals evaluated per second (whole job), inputs resident in HBM.
+``e2e``    = the same through ``snk_build_K_host`` (HOST P in, HOST K out; H2D/D2H inside the timed region).
+``roofline``: dominant integral-contraction kernel (bound "alu": plain FP64 DFMA pipe) -- algorithmic flops of its
+launch (DESIGN.md flop model) / its CUDA-event duration inside the timed region / measured DFMA peak of this GPU.
+``cpu_baseline``: the oracle, as it stands, on the host cores, on a bounded sample (whole root cells, R13).
+
+N > 1 (torchrun): the grid's root cells are dealt to ranks by Alg. 2 (greedy LPT), every rank
+builds its partial K and one NCCL all-reduce (Alg. 1 line 13) sums them -- strong scaling of one build.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "sn-K build: contracted 3c-CP integrals per second (snk_build_K wall time also reported as ms_per_step)"
+UNIT = "integrals/s"
+
+
+def _workload_name(cfg, w):
+    return "cfg%d %s: %d atoms, %d shells, %d functions, grid %s = %d points, eps=%g" % (
+        cfg, w.name, len(w.atoms_z), w.basis.nshells, w.basis.nbf, "x".join(map(str, w.grid_shape)), w.points.shape[0], w.eps)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.p = None
+
+    def _read(self):
+        for line in self.p.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        sm, mx, reasons = [], [], set()
+        for (t, line) in self.rows:
+            if t < t0 or t > t1 + 0.2:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except Exception:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in timed region"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle_sample(w, target_s=15.0, first_frac=0.01):
+    """Oracle (as it stands) on a bounded whole-root-cell sample sized for ~target_s of host time."""
+    from oracle import oracle as orc
+    from paper_2303_14280_b200.dist import root_cell_sample
+    o = orc.Oracle(w.basis)
+
+    def run(frac):
+        m = root_cell_sample(w.points, w.batch_cell, frac) if frac < 1.0 else np.ones(w.points.shape[0], dtype=bool)
+        o.set_grid(w.points[m], w.weights[m], eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
+        t = time.time()
+        o.build_K(w.P)
+        dt = time.time() - t
+        st = o.stats()
+        return dt, st, int(m.sum())
+
+    dt, st, npt = run(first_frac)
+    rate = st["n_pairpoints"] / max(dt, 1e-6)
+    # second run sized from the first one's rate (pair-points per point assumed uniform)
+    frac = min(1.0, first_frac * target_s / max(dt, 1e-3))
+    if frac > 1.5 * first_frac:
+        dt, st, npt = run(frac)
+    return dict(value=st["n_int_contracted"] / dt, unit=UNIT, cores=st["threads"], kind="oracle",
+                sample="whole root cells (R13 hash order): %d of %d points (%.2f%%), %.3g contracted integrals, %.2f s; "
+                       "oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % (npt, w.points.shape[0], 100.0 * npt / w.points.shape[0],
+                                                                                  st["n_int_contracted"], dt),
+                seconds=dt, n_int=st["n_int_contracted"])
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, same config/metric; each step = a bounded sample."""
+    if rank != 0:
+        return
+    from paper_2303_14280_b200 import inputs
+    w = inputs.make_workload(args.config, grid=args.grid, device="cpu" if args.config in (1, 2, 5) else _gen_device())
+    per_step = max(2.0, 120.0 / max(1, args.steps + args.warmup))
+    res = []
+    for i in range(args.warmup + args.steps):
+        r = time_oracle_sample(w, target_s=min(per_step, 20.0))
+        if i >= args.warmup:
+            res.append(r)
+    n_int = sum(r["n_int"] for r in res)
+    secs = sum(r["seconds"] for r in res)
+    val = n_int / secs
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(args.config, w), "sample": res[-1]["sample"]},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": res[-1]["cores"], "kind": "oracle", "sample": res[-1]["sample"]},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def _gen_device():
+    try:
+        import torch
+        return "cuda" if torch.cuda.is_available() else "cpu"
+    except Exception:
+        return "cpu"
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
+    ap.add_argument("--grid", type=lambda s: tuple(int(x) for x in s.split(",")), default=None, help="override n_r,n_theta,n_phi")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--workspace-gb", type=float, default=None)
+    ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
+                    help="N>1: 'replicas' = every rank builds K for its own density (independent problems, no collective, weak scaling); "
+                         "'shard' = root cells dealt to ranks + NCCL all-reduce of K (Alg. 1/2, strong scaling)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2303_14280_b200 import inputs, snk
+    from paper_2303_14280_b200.dist import all_reduce_K, shard_points
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    snk.load()
+
+    # ---- synthetic workload (seeded, DESIGN.md recipe); the grid generator runs on the GPU for speed ----
+    w = inputs.make_workload(args.config, grid=args.grid, device=str(dev))
+    shard = world > 1 and args.multi == "shard"
+    mine = shard_points(w.points, w.batch_cell, rank, world) if shard else np.ones(w.points.shape[0], dtype=bool)
+    if world > 1 and not shard:       # independent problem per rank: its own density matrix, same molecule and grid
+        rng = np.random.Generator(np.random.PCG64(inputs.SEED_BASE + 1000 * rank + args.config))
+        C = rng.standard_normal((w.basis.nbf, max(1, w.basis.nbf // 5))) / np.sqrt(max(1, w.basis.nbf // 5))
+        w.P = 0.5 * (C @ C.T + (C @ C.T).T)
+    pts = torch.as_tensor(np.ascontiguousarray(w.points[mine]), device=dev)
+    wts = torch.as_tensor(np.ascontiguousarray(w.weights[mine]), device=dev)
+    P = torch.as_tensor(w.P, device=dev)
+    K = torch.empty_like(P)
+    s = snk.Snk(w.basis)
+    s.set_option("eps", w.eps); s.set_option("batch_cell", w.batch_cell); s.set_option("batch_max", w.batch_max)
+    if args.workspace_gb:
+        s.set_option("workspace_gb", args.workspace_gb)
+    dfma_peak, dmma_peak = snk.measure_fp64_peak(5)
+    s.set_grid(pts, wts)
+    set_grid_ms = s.stats()["ms_set_grid"]
+
+    def step():
+        s.build_K(P, K)
+        if shard:
+            all_reduce_K(K)             # Alg. 1 line 13
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    st = s.stats()            # per-stage CUDA-event times of the LAST timed step (recorded inside the timed region)
+    clocks = sampler.stop(t0, t1) if sampler else None
+
+    # ---- e2e: host P -> host K through snk_build_K_host ----
+    Ph = torch.as_tensor(w.P).pin_memory()
+    Kh = torch.empty_like(Ph).pin_memory()
+    s.build_K_host(Ph, Kh)
+    barrier()
+    te0 = time.time()
+    for _ in range(args.steps):
+        if world == 1:
+            s.build_K_host(Ph, Kh)
+        else:
+            P.copy_(Ph, non_blocking=True)
+            step()
+            Kh.copy_(K, non_blocking=True)
+            torch.cuda.synchronize(dev)
+    barrier()
+    e2e_s = time.time() - te0
+
+    # ---- aggregate over ranks: max time, sum of work ----
+    n_int = st["n_int_contracted"]
+    agg = torch.tensor([ms, e2e_s, n_int, st["n_int_primitive"], st["n_pairpoints"], float(st["n_launches"])], dtype=torch.float64, device=dev)
+    if world > 1:
+        mx = agg.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = agg.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms, e2e_s = float(mx[0]), float(mx[1])
+        n_int, n_prim, n_pp, n_launch = float(sm[2]), float(sm[3]), float(sm[4]), float(sm[5])
+    else:
+        n_prim, n_pp, n_launch = st["n_int_primitive"], st["n_pairpoints"], float(st["n_launches"])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = n_int * args.steps / (ms * 1e-3)
+    nbytes = w.P.nbytes
+    # dominant integral kernel of the last timed step
+    cls = int(np.argmax(st["ms_G_class"]))
+    k_ms = st["ms_G_class"][cls]
+    k_flops = st["flops_class"][cls]
+    achieved = k_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
+    all_ms = sum(st["ms_G_class"])
+    roofline = {"bound": "alu", "kernel": "k_integrals<%s>" % snk.CLASS_NAMES[cls], "achieved": achieved, "peak": dfma_peak, "unit": "TFLOP/s",
+                "frac": achieved / dfma_peak if dfma_peak else None, "traffic": None,
+                "peak_source": "measured on this GPU by snk_measure_fp64_peak (register-resident DFMA loop); nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2",
+                "flops_per_launch": k_flops, "ms_per_launch": k_ms,
+                "all_integral_kernels": {"achieved": st["flops_integral"] / (all_ms * 1e-3) * 1e-12 if all_ms > 0 else 0.0, "ms": all_ms,
+                                         "flops": st["flops_integral"], "share_of_step": all_ms / st["ms_build"] if st["ms_build"] else None},
+                "gemm_dmma": {"peak": dmma_peak, "achieved": st["flops_gemm"] / ((st["ms_F"] + st["ms_Kt"] + 1e-12) * 1e-3) * 1e-12,
+                              "ms_F": st["ms_F"], "ms_Kt": st["ms_Kt"]},
+                "flop_model": "far-field (asymptotic Boys) instruction count of the kernel templates, FMA = 2 (DESIGN.md)"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(args.config, w), "l2": "working set (Phi, F, G slabs) far larger than the 126 MB L2; no flush needed",
+                       "parallelism": "1 GPU" if world == 1 else ("root cells -> %d ranks by Alg. 2 LPT, NCCL all-reduce of K per build" % world if shard else "%d independent replicas (own density each), no collective" % world),
+                       "batch_cell": w.batch_cell, "batch_max": w.batch_max, "n_int_per_step": n_int, "n_int_primitive_per_step": n_prim,
+                       "n_pairpoints_per_step": n_pp},
+            "clocks": clocks,
+            "e2e": {"value": n_int * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                    "ms_per_step": 1e3 * e2e_s / args.steps},
+            "gpu_launches": int(n_launch * args.steps),
+            "roofline": roofline,
+            "build": {"ms_build_last": st["ms_build"], "ms_screen": st["ms_screen"], "ms_colloc": st["ms_colloc"], "ms_F": st["ms_F"],
+                      "ms_G": st["ms_G"], "ms_Kt": st["ms_Kt"], "ms_sym": st["ms_sym"], "ms_G_class": dict(zip(snk.CLASS_NAMES, st["ms_G_class"])),
+                      "set_grid_ms": set_grid_ms, "nbatch": st["nbatch"], "npair_sig": st["npair_sig"], "sum_V": st["sum_V"],
+                      "nsuper": st["nsuper"], "fp64_peak_tflops": {"dfma": dfma_peak, "dmma": dmma_peak},
+                      "whole_build_fp64_frac": (st["flops_integral"] + st["flops_gemm"]) / (st["ms_build"] * 1e-3) * 1e-12 / dfma_peak}}
+    if not args.no_cpu_baseline:
+        cb = time_oracle_sample(w, target_s=args.cpu_seconds)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

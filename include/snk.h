@@ -67,6 +67,8 @@ typedef struct snk_stats {
   double ms_build;          /* whole snk_build_K on the stream                                       */
   double ms_G_class[10];    /* a5 per (l_a,l_b) class, order (0,0),(1,0),(1,1),(2,0)...(3,3)         */
   double n_int_class[10];   /* contracted integrals per class                                        */
+  double flops_class[10];   /* flop model per class                                                  */
+  int64_t n_launches;       /* kernels of this library launched by the last snk_build_K              */
 } snk_stats;
 
 /* ---- snk_create: the basis set "B" of Alg. 1 -------------------------------------

@@ -63,6 +63,7 @@ struct snk_ctx {
   int64_t nprimpair = 0;
   int cls_beg[kNumClasses + 1] = {0};
   double gemm_flops = 0.0;
+  int64_t n_launches = 0;
   // timing
   std::vector<cudaEvent_t> ev_pool;
   struct Span { int stage; int cls; int e0, e1; };
@@ -309,7 +310,7 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
   if (e == cudaSuccess) e = ctx->d_rcut2.reserve(nshells);
   if (e == cudaSuccess) e = ctx->d_phimax.reserve(1);
   if (e == cudaSuccess) e = ctx->d_Fmax.reserve(nshells);
-  if (e == cudaSuccess) e = ctx->d_stats.reserve(16);
+  if (e == cudaSuccess) e = ctx->d_stats.reserve(32);
   if (e == cudaSuccess) {
     std::vector<double> cf(2 * kNumClasses);
     for (int la = 0; la < 4; ++la)
@@ -498,7 +499,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   cudaStream_t s = (cudaStream_t)stream_;
   ctx->last_stream = s;
   ctx->stats_valid = false; ctx->have_build = false;
-  ctx->spans.clear(); ctx->ev_used = 0; ctx->gemm_flops = 0.0;
+  ctx->spans.clear(); ctx->ev_used = 0; ctx->gemm_flops = 0.0; ctx->n_launches = 0;
   const int nbf = ctx->nbf, nsh = ctx->nsh, nb = ctx->nbatch;
   const ShellTab tab = ctx->tab();
   CK(cudaEventRecord(ctx->ev_b0, s));
@@ -550,6 +551,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   CK(run_prim_fill(npair, tab, ctx->d_pairs.p, ctx->d_prims.p, 1e-4 * ctx->eps, (const double*)ctx->d_Fmax.p, (const double*)ctx->d_phimax.p, s));
   CK(cudaMemsetAsync(ctx->d_vmask.p, 0, (size_t)nb * ctx->vstride * sizeof(uint32_t), s));
   CK(run_vmask(nb, npair, ctx->d_pairs.p, ctx->d_pairAt.p, ctx->d_FtsT.p, nsh, ctx->d_phit.p, ctx->eps, ctx->d_vmask.p, ctx->vstride, s));
+  ctx->n_launches += 7;
   span_end(sp);
 
   CK(cudaMemsetAsync(ctx->d_Kt.p, 0, (size_t)nbf * nbf * sizeof(double), s));
@@ -577,6 +579,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
       if (ip.pend <= ip.pbeg) continue;
       auto spc = span_begin(ST_COUNT, c);
       CK(launch_integrals(c, ip, s));
+      ctx->n_launches += 1;
       span_end(spc);
     }
     span_end(sp);
@@ -584,11 +587,13 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     sp = span_begin(ST_KT, -1);
     CK(gemm_f64(true, nbf, nbf, su.nslots, ctx->d_Phi.p, ctx->ld, ctx->d_G.p, ctx->ld, ctx->d_Kt.p, nbf, true, ctx->gw.p + su.slot0, s));
     ctx->gemm_flops += 2.0 * nbf * (double)su.nslots * nbf;
+    ctx->n_launches += 3;   // collocation, F GEMM, Kt GEMM
     span_end(sp);
   }
   // ---- a7 ----
   sp = span_begin(ST_SYM, -1);
   CK(run_symmetrise(nbf, ctx->d_Kt.p, K, s));
+  ctx->n_launches += 1;
   span_end(sp);
   CK(cudaEventRecord(ctx->ev_b1, s));
   ctx->have_build = true;
@@ -618,16 +623,17 @@ int snk_get_stats(snk_ctx* ctx, snk_stats* out) {
   st.nsuper = (int64_t)ctx->supers.size();
   if (ctx->have_build && !ctx->stats_valid) {
     st.npair_sig = ctx->npair_sig; st.nprimpair = ctx->nprimpair; st.flops_gemm = ctx->gemm_flops;
-    double h[16] = {0};
+    double h[32] = {0};
     if (ctx->nbatch > 0 && ctx->npair_sig > 0) {
-      CK(cudaMemsetAsync(ctx->d_stats.p, 0, 16 * sizeof(double), s));
+      CK(cudaMemsetAsync(ctx->d_stats.p, 0, 32 * sizeof(double), s));
       CK(run_vstats(ctx->nbatch, ctx->npair_sig, ctx->d_pairs.p, ctx->tab(), ctx->d_bn.p, ctx->d_vmask.p, ctx->vstride, ctx->d_cflops.p,
                     ctx->d_cflops.p + kNumClasses, ctx->d_stats.p, s));
-      CK(cudaMemcpyAsync(h, ctx->d_stats.p, 16 * sizeof(double), cudaMemcpyDeviceToHost, s));
+      CK(cudaMemcpyAsync(h, ctx->d_stats.p, 32 * sizeof(double), cudaMemcpyDeviceToHost, s));
       CK(cudaStreamSynchronize(s));
     }
     st.sum_V = (int64_t)h[0]; st.n_pairpoints = h[1]; st.n_int_contracted = h[2]; st.n_int_primitive = h[3];
-    for (int c = 0; c < kNumClasses; ++c) st.n_int_class[c] = h[4 + c];
+    for (int c = 0; c < kNumClasses; ++c) { st.n_int_class[c] = h[4 + c]; st.flops_class[c] = h[16 + c]; }
+    st.n_launches = ctx->n_launches;
     st.flops_integral = h[14];
     double acc[ST_COUNT] = {0};
     for (int c = 0; c < kNumClasses; ++c) st.ms_G_class[c] = 0.0;

@@ -8,6 +8,8 @@
 // CTA tile 128 x 128 x 16, 8 warps (2 x 4), warp tile 64 x 32 = 8 x 4 m8n8 fragments, accumulators in registers.
 // Shared tiles are stored k-major with row stride 132 doubles so that the m8n8k4 fragment loads
 // (thread (g = lane/4, t = lane%4) reads [k = t][m = g]) hit 16 distinct 8-byte banks per half-warp.
+#include <algorithm>
+
 #include "snk_internal.h"
 
 namespace snk {
@@ -67,7 +69,7 @@ __device__ __forceinline__ void store_tile(const double (&r)[8], double* __restr
 template <bool TRANSB>
 __global__ void __launch_bounds__(NT) k_gemm_f64(int64_t M, int64_t N, int64_t K, const double* __restrict__ A, int64_t lda,
                                                  const double* __restrict__ B, int64_t ldb, double* __restrict__ C, int64_t ldc,
-                                                 bool beta, const double* __restrict__ kscale) {
+                                                 bool beta, const double* __restrict__ kscale, int64_t kchunk) {
   extern __shared__ __align__(16) double smem_gemm[];
   double (*As)[BK * LDS] = reinterpret_cast<double (*)[BK * LDS]>(smem_gemm);
   double (*Bs)[BK * LDS] = reinterpret_cast<double (*)[BK * LDS]>(smem_gemm + 2 * BK * LDS);
@@ -82,10 +84,14 @@ __global__ void __launch_bounds__(NT) k_gemm_f64(int64_t M, int64_t N, int64_t K
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
+  // split-K: this CTA contracts k in [kbeg, kend); partial results are RED-added (only used with beta = true)
+  const int64_t kbeg = (int64_t)blockIdx.z * kchunk;
+  const int64_t kend = min(K, kbeg + kchunk);
+  const bool atomic_out = gridDim.z > 1;
   double ra[8], rb[8];
-  const int64_t nk = (K + BK - 1) / BK;
-  load_tile<true>(ra, A, lda, m0, M, 0, K, kscale, tid);
-  load_tile<TRANSB>(rb, B, ldb, n0, N, 0, K, nullptr, tid);
+  const int64_t nk = kend > kbeg ? (kend - kbeg + BK - 1) / BK : 0;
+  load_tile<true>(ra, A, lda, m0, M, kbeg, kend, kscale, tid);
+  load_tile<TRANSB>(rb, B, ldb, n0, N, kbeg, kend, nullptr, tid);
   store_tile<true>(ra, As[0], tid);
   store_tile<TRANSB>(rb, Bs[0], tid);
   __syncthreads();
@@ -93,8 +99,8 @@ __global__ void __launch_bounds__(NT) k_gemm_f64(int64_t M, int64_t N, int64_t K
   for (int64_t kt = 0; kt < nk; ++kt) {
     const int cur = kt & 1;
     if (kt + 1 < nk) {
-      load_tile<true>(ra, A, lda, m0, M, (kt + 1) * BK, K, kscale, tid);
-      load_tile<TRANSB>(rb, B, ldb, n0, N, (kt + 1) * BK, K, nullptr, tid);
+      load_tile<true>(ra, A, lda, m0, M, kbeg + (kt + 1) * BK, kend, kscale, tid);
+      load_tile<TRANSB>(rb, B, ldb, n0, N, kbeg + (kt + 1) * BK, kend, nullptr, tid);
     }
     const double* as = As[cur] + wm * 64 + g;
     const double* bs = Bs[cur] + wn * 32 + g;
@@ -126,8 +132,13 @@ __global__ void __launch_bounds__(NT) k_gemm_f64(int64_t M, int64_t N, int64_t K
     for (int j = 0; j < 4; ++j) {
       const int64_t col = n0 + wn * 32 + j * 8 + 2 * t;
       double* c = C + row * ldc + col;
-      if (col < N) c[0] = beta ? c[0] + acc[i][j][0] : acc[i][j][0];
-      if (col + 1 < N) c[1] = beta ? c[1] + acc[i][j][1] : acc[i][j][1];
+      if (atomic_out) {
+        if (col < N) atomicAdd(c, acc[i][j][0]);
+        if (col + 1 < N) atomicAdd(c + 1, acc[i][j][1]);
+      } else {
+        if (col < N) c[0] = beta ? c[0] + acc[i][j][0] : acc[i][j][0];
+        if (col + 1 < N) c[1] = beta ? c[1] + acc[i][j][1] : acc[i][j][1];
+      }
     }
   }
 }
@@ -137,6 +148,17 @@ cudaError_t gemm_f64(bool transB, int64_t M, int64_t N, int64_t K, const double*
                      double* C, int64_t ldc, bool beta, const double* kscale, cudaStream_t s) {
   if (M <= 0 || N <= 0) return cudaSuccess;
   dim3 grid((unsigned)((N + BN - 1) / BN), (unsigned)((M + BM - 1) / BM));
+  // split-K when the output is too small to fill the GPU (the Kt contraction: M = N = nbf, K = grid points)
+  int64_t kchunk = K > 0 ? K : 1;
+  if (beta && K > 0) {
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    const int64_t ctas = (int64_t)grid.x * grid.y;
+    int64_t split = (2 * sms + ctas - 1) / ctas;
+    split = std::max<int64_t>(1, std::min<int64_t>(split, K / (8 * BK)));
+    kchunk = ((K + split - 1) / split + BK - 1) / BK * BK;
+    grid.z = (unsigned)((K + kchunk - 1) / kchunk);
+  }
   constexpr int smem = 4 * BK * LDS * (int)sizeof(double);
   static bool attr_set = false;
   if (!attr_set) {
@@ -144,8 +166,8 @@ cudaError_t gemm_f64(bool transB, int64_t M, int64_t N, int64_t K, const double*
     cudaFuncSetAttribute(k_gemm_f64<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     attr_set = true;
   }
-  if (transB) k_gemm_f64<true><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale);
-  else k_gemm_f64<false><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale);
+  if (transB) k_gemm_f64<true><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale, kchunk);
+  else k_gemm_f64<false><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale, kchunk);
   return cudaGetLastError();
 }
 

@@ -387,7 +387,7 @@ __global__ void k_vmask(int npair, const PairRec* __restrict__ pairs, const doub
 }
 
 // counters for snk_stats: out[0]=sum|V_j|, [1]=pair-points, [2]=contracted integrals, [3]=primitive integrals,
-// [4..13] contracted integrals per class, [14] flop model
+// [4..13] contracted integrals per class, [14] flop model, [16..25] flop model per class
 __global__ void k_vstats(int npair, const PairRec* __restrict__ pairs, ShellTab sh, const int32_t* __restrict__ bn,
                          const uint32_t* __restrict__ vmask, int64_t vstride, const double* __restrict__ class_flops_prim,
                          const double* __restrict__ class_flops_contr, double* __restrict__ out) {
@@ -404,7 +404,9 @@ __global__ void k_vstats(int npair, const PairRec* __restrict__ pairs, ShellTab 
   atomicAdd(out + 2, nq * nc);
   atomicAdd(out + 3, nq * nc * r.nprim);
   atomicAdd(out + 4 + cls, nq * nc);
-  atomicAdd(out + 14, nq * (class_flops_prim[cls] * r.nprim + class_flops_contr[cls]));
+  const double fl = nq * (class_flops_prim[cls] * r.nprim + class_flops_contr[cls]);
+  atomicAdd(out + 14, fl);
+  atomicAdd(out + 16 + cls, fl);
 }
 
 // ------------------------------------------------------------------------------------------------------------

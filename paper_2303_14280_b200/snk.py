@@ -30,7 +30,8 @@ class SnkStats(C.Structure):
                 ("n_pairpoints", C.c_double), ("n_int_contracted", C.c_double), ("n_int_primitive", C.c_double),
                 ("flops_integral", C.c_double), ("flops_gemm", C.c_double), ("ms_set_grid", C.c_double), ("ms_screen", C.c_double),
                 ("ms_colloc", C.c_double), ("ms_F", C.c_double), ("ms_G", C.c_double), ("ms_Kt", C.c_double), ("ms_sym", C.c_double),
-                ("ms_build", C.c_double), ("ms_G_class", C.c_double * 10), ("n_int_class", C.c_double * 10)]
+                ("ms_build", C.c_double), ("ms_G_class", C.c_double * 10), ("n_int_class", C.c_double * 10),
+                ("flops_class", C.c_double * 10), ("n_launches", C.c_int64)]
 
     def asdict(self):
         d = {}
