@@ -52,14 +52,14 @@ struct snk_ctx {
   DevBuf<double> d_Phi, d_F, d_G;
   // build state
   bool have_build = false, stats_valid = false;
-  DevBuf<double> d_absP, d_Ftf, d_FtsT, d_Kt, d_pairAt, d_Pin, d_Kout, d_stats, d_cflops;
-  DevBuf<int32_t> d_flag, d_np, d_pos, d_ppos;
-  DevBuf<PairRec> d_pairs;
-  DevBuf<PrimPair> d_prims;
+  DevBuf<double> d_absP, d_Ftf, d_FtsT, d_Kt, d_Pin, d_Kout, d_stats, d_cflops;
+  DevBuf<int32_t> d_flag, d_np, d_pos, d_ppos;     // per candidate pair: #units, is-pair flag, and their exclusive scans
+  DevBuf<unsigned char> d_units;                    // [nunit][kUnitBytes]
+  DevBuf<UnitMeta> d_meta;                          // [nunit]
   DevBuf<uint32_t> d_vmask;
   DevBuf<char> d_tmp;
   int64_t vstride = 0;
-  int npair_sig = 0;
+  int npair_sig = 0, nunit = 0;
   int64_t nprimpair = 0;
   int cls_beg[kNumClasses + 1] = {0};
   double gemm_flops = 0.0;
@@ -109,11 +109,13 @@ cudaError_t upload(DevBuf<T>& b, const std::vector<T>& v) {
   return e;
 }
 
-// F_m(x_i) table for the Taylor path of the device Boys function (R15): top order by the all-positive series in
-// long double, lower orders by downward recursion.  Own generator of the library (the oracle has its own code).
+// Tables for the Taylor path of the device Boys function (R15, layout in snk_os.cuh): for every top order L the scaled
+// derivatives F_{L+k}(x_i)/k!, k = 0..7, and e^{-x_i}.  F at the highest order by the all-positive series in long double,
+// lower orders by downward recursion.  Own generator of the library (the oracle has its own code).
 std::vector<double> make_boys_table() {
-  std::vector<double> t((size_t)kBoysRows * kBoysStride, 0.0);
-  const int mtop = kBoysStride - 1;
+  std::vector<double> t((size_t)(kBoysLmax + 1) * kBoysRows * kBoysStride, 0.0);
+  const int mtop = kBoysLmax + 7;
+  std::vector<long double> F(mtop + 1);
   for (int i = 0; i < kBoysRows; ++i) {
     const long double x = (long double)i * (long double)kBoysDelta;
     const long double ex = expl(-x);
@@ -123,11 +125,13 @@ std::vector<double> make_boys_table() {
       sum += term;
       if (term < 1e-22L * sum) break;
     }
-    long double F = ex * sum;
-    t[(size_t)i * kBoysStride + mtop] = (double)F;
-    for (int m = mtop; m >= 1; --m) {
-      F = (2.0L * x * F + ex) / (2 * m - 1);
-      t[(size_t)i * kBoysStride + m - 1] = (double)F;
+    F[mtop] = ex * sum;
+    for (int m = mtop; m >= 1; --m) F[m - 1] = (2.0L * x * F[m] + ex) / (2 * m - 1);
+    for (int L = 0; L <= kBoysLmax; ++L) {
+      double* row = &t[((size_t)L * kBoysRows + i) * kBoysStride];
+      long double fact = 1.0L;
+      for (int k = 0; k < 8; ++k) { if (k > 0) fact *= k; row[k] = (double)(F[L + k] / fact); }
+      row[8] = (double)ex;
     }
   }
   return t;
@@ -230,10 +234,10 @@ void snk_destroy(snk_ctx* ctx) {
   ctx->gx.release(); ctx->gy.release(); ctx->gz.release(); ctx->gw.release(); ctx->d_PhiTf.release(); ctx->d_phit.release();
   ctx->slot_src.release(); ctx->d_bslot.release(); ctx->d_bn.release(); ctx->d_bmask.release(); ctx->d_phimax.release();
   ctx->d_Fmax.release(); ctx->d_tiles.release(); ctx->d_Phi.release(); ctx->d_F.release(); ctx->d_G.release();
-  ctx->d_absP.release(); ctx->d_Ftf.release(); ctx->d_FtsT.release(); ctx->d_Kt.release(); ctx->d_pairAt.release();
+  ctx->d_absP.release(); ctx->d_Ftf.release(); ctx->d_FtsT.release(); ctx->d_Kt.release();
   ctx->d_Pin.release(); ctx->d_Kout.release(); ctx->d_stats.release(); ctx->d_cflops.release();
-  ctx->d_flag.release(); ctx->d_np.release(); ctx->d_pos.release(); ctx->d_ppos.release(); ctx->d_pairs.release();
-  ctx->d_prims.release(); ctx->d_vmask.release(); ctx->d_tmp.release();
+  ctx->d_flag.release(); ctx->d_np.release(); ctx->d_pos.release(); ctx->d_ppos.release(); ctx->d_units.release();
+  ctx->d_meta.release(); ctx->d_vmask.release(); ctx->d_tmp.release();
   for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
   for (cudaEvent_t e : {ctx->ev_b0, ctx->ev_b1, ctx->ev_g0, ctx->ev_g1}) if (e) cudaEventDestroy(e);
   delete ctx;
@@ -506,7 +510,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   if (nb == 0) {
     CK(cudaMemsetAsync(K, 0, (size_t)nbf * nbf * sizeof(double), s));
     CK(cudaEventRecord(ctx->ev_b1, s));
-    ctx->npair_sig = 0; ctx->nprimpair = 0; ctx->have_build = true;
+    ctx->npair_sig = 0; ctx->nunit = 0; ctx->nprimpair = 0; ctx->have_build = true;
     return SNK_OK;
   }
   auto span_begin = [&](int stage, int cls) { snk_ctx::Span sp{stage, cls, ctx->new_event(), -1}; cudaEventRecord(ctx->ev_pool[sp.e0], s); return sp; };
@@ -539,19 +543,19 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   for (int c = 0; c < kNumClasses; ++c)
     if (ctx->cand.off[c] < ncand) CK(cudaMemcpyAsync(&h_cls[c], ctx->d_pos.p + ctx->cand.off[c], 4, cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
-  const int npair = h_last[0] + h_last[1];
-  const int64_t nprim = (int64_t)h_last[2] + h_last[3];
-  for (int c = 0; c < kNumClasses; ++c) ctx->cls_beg[c] = ctx->cand.off[c] < ncand ? h_cls[c] : npair;
-  ctx->cls_beg[kNumClasses] = npair;
-  ctx->npair_sig = npair; ctx->nprimpair = nprim;
-  ctx->vstride = (npair + 31) / 32 + 1;
-  CK(ctx->d_pairs.reserve(std::max(npair, 1))); CK(ctx->d_pairAt.reserve(std::max(npair, 1))); CK(ctx->d_prims.reserve(std::max<int64_t>(nprim, 1)));
+  const int nunit = h_last[0] + h_last[1];
+  const int npair = h_last[2] + h_last[3];
+  for (int c = 0; c < kNumClasses; ++c) ctx->cls_beg[c] = ctx->cand.off[c] < ncand ? h_cls[c] : nunit;
+  ctx->cls_beg[kNumClasses] = nunit;
+  ctx->npair_sig = npair; ctx->nunit = nunit;
+  ctx->vstride = (nunit + 31) / 32 + 1;
+  CK(ctx->d_units.reserve((size_t)std::max(nunit, 1) * kUnitBytes)); CK(ctx->d_meta.reserve(std::max(nunit, 1)));
   CK(ctx->d_vmask.reserve((size_t)nb * ctx->vstride));
-  CK(run_pair_compact(ctx->cand, tab, ctx->d_flag.p, ctx->d_pos.p, ctx->d_ppos.p, ctx->d_Atil.p, ctx->d_pairs.p, ctx->d_pairAt.p, s));
-  CK(run_prim_fill(npair, tab, ctx->d_pairs.p, ctx->d_prims.p, 1e-4 * ctx->eps, (const double*)ctx->d_Fmax.p, (const double*)ctx->d_phimax.p, s));
+  CK(run_unit_fill(ctx->cand, tab, ctx->d_flag.p, ctx->d_pos.p, ctx->d_Atil.p, 1e-4 * ctx->eps, (const double*)ctx->d_Fmax.p,
+                   (const double*)ctx->d_phimax.p, ctx->d_units.p, ctx->d_meta.p, s));
   CK(cudaMemsetAsync(ctx->d_vmask.p, 0, (size_t)nb * ctx->vstride * sizeof(uint32_t), s));
-  CK(run_vmask(nb, npair, ctx->d_pairs.p, ctx->d_pairAt.p, ctx->d_FtsT.p, nsh, ctx->d_phit.p, ctx->eps, ctx->d_vmask.p, ctx->vstride, s));
-  ctx->n_launches += 7;
+  CK(run_vmask(nb, nunit, ctx->d_meta.p, ctx->d_FtsT.p, nsh, ctx->d_phit.p, ctx->eps, ctx->d_vmask.p, ctx->vstride, s));
+  ctx->n_launches += 6;
   span_end(sp);
 
   CK(cudaMemsetAsync(ctx->d_Kt.p, 0, (size_t)nbf * nbf * sizeof(double), s));
@@ -573,7 +577,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     IntParams ip;
     ip.gx = ctx->gx.p; ip.gy = ctx->gy.p; ip.gz = ctx->gz.p; ip.F = ctx->d_F.p; ip.G = ctx->d_G.p; ip.ld = ctx->ld; ip.slot0 = su.slot0;
     ip.tiles = ctx->d_tiles.p + su.t0; ip.ntiles = ntiles; ip.vmask = ctx->d_vmask.p; ip.vstride = ctx->vstride;
-    ip.pairs = ctx->d_pairs.p; ip.prims = ctx->d_prims.p; ip.boys = ctx->d_boys.p;
+    ip.units = ctx->d_units.p; ip.meta = ctx->d_meta.p; ip.boys = ctx->d_boys.p;
     for (int c = 0; c < kNumClasses; ++c) {
       ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1];
       if (ip.pend <= ip.pbeg) continue;
@@ -622,11 +626,18 @@ int snk_get_stats(snk_ctx* ctx, snk_stats* out) {
   st.npts = ctx->npts; st.npts_kept = ctx->npts_kept; st.nbatch = ctx->nbatch; st.sum_B = ctx->sum_B; st.sum_B_fn = ctx->sum_B_fn;
   st.nsuper = (int64_t)ctx->supers.size();
   if (ctx->have_build && !ctx->stats_valid) {
+    if (ctx->nunit > 0) {      // primitive pairs kept (R14): from the unit metadata, off the timed path
+      std::vector<UnitMeta> hm(ctx->nunit);
+      CK(cudaMemcpyAsync(hm.data(), ctx->d_meta.p, hm.size() * sizeof(UnitMeta), cudaMemcpyDeviceToHost, s));
+      CK(cudaStreamSynchronize(s));
+      ctx->nprimpair = 0;
+      for (const UnitMeta& m : hm) ctx->nprimpair += m.nprim_first & 0xff;
+    }
     st.npair_sig = ctx->npair_sig; st.nprimpair = ctx->nprimpair; st.flops_gemm = ctx->gemm_flops;
     double h[32] = {0};
-    if (ctx->nbatch > 0 && ctx->npair_sig > 0) {
+    if (ctx->nbatch > 0 && ctx->nunit > 0) {
       CK(cudaMemsetAsync(ctx->d_stats.p, 0, 32 * sizeof(double), s));
-      CK(run_vstats(ctx->nbatch, ctx->npair_sig, ctx->d_pairs.p, ctx->tab(), ctx->d_bn.p, ctx->d_vmask.p, ctx->vstride, ctx->d_cflops.p,
+      CK(run_vstats(ctx->nbatch, ctx->nunit, ctx->d_meta.p, ctx->tab(), ctx->d_bn.p, ctx->d_vmask.p, ctx->vstride, ctx->d_cflops.p,
                     ctx->d_cflops.p + kNumClasses, ctx->d_stats.p, s));
       CK(cudaMemcpyAsync(h, ctx->d_stats.p, 32 * sizeof(double), cudaMemcpyDeviceToHost, s));
       CK(cudaStreamSynchronize(s));
@@ -689,10 +700,10 @@ int snk_export_lists(snk_ctx* ctx, int64_t* sizes, int64_t* batch_off, int64_t* 
   } else if (B_off) B_off[0] = 0;
   if ((V_off || V_pairs) && nb > 0) {
     if (!ctx->have_build) FAIL(SNK_ESTATE, "snk_export_lists: V_j need a prior snk_build_K");
-    const int np = ctx->npair_sig;
-    std::vector<PairRec> hp(std::max(np, 1));
+    const int np = ctx->nunit;
+    std::vector<UnitMeta> hp(std::max(np, 1));
     std::vector<uint32_t> hv((size_t)nb * ctx->vstride);
-    if (np > 0) CK(cudaMemcpy(hp.data(), ctx->d_pairs.p, (size_t)np * sizeof(PairRec), cudaMemcpyDeviceToHost));
+    if (np > 0) CK(cudaMemcpy(hp.data(), ctx->d_meta.p, (size_t)np * sizeof(UnitMeta), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(hv.data(), ctx->d_vmask.p, hv.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost));
     int64_t o = 0;
     std::vector<std::pair<int32_t, int32_t>> tmp;
@@ -700,7 +711,7 @@ int snk_export_lists(snk_ctx* ctx, int64_t* sizes, int64_t* batch_off, int64_t* 
       if (V_off) V_off[j] = o;
       tmp.clear();
       for (int i = 0; i < np; ++i)
-        if ((hv[(size_t)j * ctx->vstride + (i >> 5)] >> (i & 31)) & 1u)
+        if (((hv[(size_t)j * ctx->vstride + (i >> 5)] >> (i & 31)) & 1u) && ((hp[i].nprim_first >> 8) & 1))
           tmp.emplace_back(std::min(hp[i].sa, hp[i].sb), std::max(hp[i].sa, hp[i].sb));
       std::sort(tmp.begin(), tmp.end());
       for (auto& ab : tmp) { if (V_pairs) { V_pairs[2 * o] = ab.first; V_pairs[2 * o + 1] = ab.second; } ++o; }

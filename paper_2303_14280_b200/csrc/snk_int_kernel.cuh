@@ -1,64 +1,172 @@
 // snk_int_kernel.cuh -- integral-contraction kernel (row a5):  G[nu][g] += sum_{(nu,lam) in V_j} A_{nu,lam}(g) F[lam][g]
-// Eq. 38/48 via App. A.  One thread = one grid point, one CTA = one tile of
-// kTile consecutive points of one batch; all threads of a CTA walk the same V_j bit mask, so control flow is uniform.
-// The pair list of a class is sorted by (a, b): G_a / F_a stay in registers over a run of pairs sharing a.
-// A is never stored.  Included once per (LA,LB) translation unit.
+// Eq. 38/48 via App. A.  One consumer thread = one grid point, one CTA = one tile of
+// up to kTile consecutive points of one batch.  A is never stored.
+//
+// B200 design (differs from the paper's A100 kernel):
+//   * warp-specialised: warps 0..3 are consumers, warp 4 is a producer that walks the tile's V_j bit mask and streams
+//     every kept pair unit -- header + primitive pairs (<= 704 B) and the F_b rows of this tile -- into a ring of
+//     shared-memory slots with cp.async.bulk (TMA bulk copy) completing on an mbarrier; consumers never touch pair
+//     data in global memory, so the recurrences run against broadcast LDS only;
+//   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
+//     fire-and-forget RED.F64 (coalesced along the slot index);
+//   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh);
+//   * consumer warps with no point of the tile retire immediately.
+// Included once per (LA,LB) translation unit.
 #pragma once
 #include "snk_internal.h"
 #include "snk_os.cuh"
 
 namespace snk {
 
+constexpr int kConsumerWarps = kTile / 32;
+constexpr int kIntThreads = kTile + 32;
+
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : (LA + LB >= 2 ? 6 : 8); }
+__host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
+__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB); }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "SNK_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra SNK_DONE_%=;\n"
+      "bra SNK_WAIT_%=;\n"
+      "SNK_DONE_%=:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
+               "r"(bar)
+               : "memory");
+}
+
 template <int LA, int LB>
-__global__ void __launch_bounds__(kTile) k_integrals(IntParams p) {
+__global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
+  constexpr int NS = int_nslots(LA, LB), SLOT = int_slot_bytes(LB);
+  extern __shared__ __align__(128) unsigned char smem_int[];
+  const uint32_t s_base = smem_u32(smem_int);
+  const uint32_t s_full = s_base + NS * SLOT, s_empty = s_full + NS * 8;
+
   const TileRec tile = p.tiles[blockIdx.x];
-  const int t = threadIdx.x;
+  const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+  const int nw = (tile.n + 31) >> 5;                       // consumer warps that own at least one point
+  const int npad = nw << 5;
+  if (t == 0) {
+    for (int i = 0; i < NS; ++i) { mbar_init(s_full + 8 * i, 1); mbar_init(s_empty + 8 * i, nw); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int64_t col0 = tile.slot - p.slot0;
+
+  if (warp == kConsumerWarps) {
+    // ------------------------------------------------ producer warp ------------------------------------------------
+    const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
+    const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
+    const uint32_t frow = (uint32_t)npad * 8u;             // bytes of one staged F row
+    uint32_t u = 0;                                        // units issued so far
+    for (int wb = w0; wb < w1; wb += 32) {
+      const int w = wb + lane;
+      uint32_t word = w < w1 ? __ldg(mask + w) : 0u;
+      if (w == w0) word &= 0xffffffffu << (p.pbeg & 31);
+      if (w == w1 - 1 && (p.pend & 31)) word &= 0xffffffffu >> (32 - (p.pend & 31));
+      uint32_t any = __ballot_sync(~0u, word != 0u);
+      while (any) {
+        const int src = __ffs(any) - 1;
+        any &= any - 1;
+        const uint32_t bits = __shfl_sync(~0u, word, src);
+        const int n = __popc(bits);
+        const int base_pid = (wb + src) << 5;
+        for (int b0 = 0; b0 < n; b0 += NS) {               // at most NS units in flight per step: one lane per unit
+          const bool mine = lane >= b0 && lane < min(n, b0 + NS);
+          if (mine) {
+            const int pid = base_pid + (int)__fns(bits, 0, lane + 1);
+            const UnitMeta m = p.meta[pid];
+            const uint32_t uu = u + (uint32_t)(lane - b0);
+            const uint32_t slot = uu % NS, round = uu / NS;
+            if (round > 0) mbar_wait(s_empty + 8 * slot, (round - 1) & 1);
+            const uint32_t nb = 64u + (uint32_t)(m.nprim_first & 0xff) * (uint32_t)kPrimBytes;
+            const uint32_t bar = s_full + 8 * slot, dst = s_base + slot * SLOT;
+            mbar_arrive_expect_tx(bar, nb + NB * frow);
+            bulk_g2s(dst, p.units + (size_t)pid * kUnitBytes, nb, bar);
+            const double* __restrict__ Fsrc = p.F + (int64_t)m.fb * p.ld + col0;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) bulk_g2s(dst + kUnitBytes + k * (kTile * 8), Fsrc + (int64_t)k * p.ld, frow, bar);
+          }
+          u += (uint32_t)(min(n, b0 + NS) - b0);
+          __syncwarp();
+        }
+      }
+    }
+    if (lane == 0) {                                       // end-of-list sentinel: a header with fa = -1
+      const uint32_t slot = u % NS, round = u / NS;
+      if (round > 0) mbar_wait(s_empty + 8 * slot, (round - 1) & 1);
+      reinterpret_cast<volatile int32_t*>(smem_int + slot * SLOT)[0] = -1;
+      mbar_arrive(s_full + 8 * slot);
+    }
+    return;
+  }
+  if (warp >= nw) return;
+
+  // -------------------------------------------------- consumer warps --------------------------------------------------
   const bool active = t < tile.n;
   const int64_t slot = tile.slot + (active ? t : tile.n - 1);
   const double gx = p.gx[slot], gy = p.gy[slot], gz = p.gz[slot];
-  const int64_t col = slot - p.slot0;
-  const double* __restrict__ Fc = p.F + col;
-  double* __restrict__ Gc = p.G + col;
-  const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
+  const double* __restrict__ Fc = p.F + col0 + t;
+  double* __restrict__ Gc = p.G + col0 + t;
 
   int cur_fa = -1;
   double Fa[NA], Ga[NA];
 #pragma unroll
   for (int i = 0; i < NA; ++i) { Fa[i] = 0.0; Ga[i] = 0.0; }
 
-  const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
-  for (int w = w0; w < w1; ++w) {
-    uint32_t bits = __ldg(mask + w);
-    if (w == w0) bits &= 0xffffffffu << (p.pbeg & 31);
-    if (w == w1 - 1 && (p.pend & 31)) bits &= 0xffffffffu >> (32 - (p.pend & 31));
-    while (bits) {
-      const int pid = (w << 5) + (__ffs(bits) - 1);
-      bits &= bits - 1;
-      const PairRec* __restrict__ pr = p.pairs + pid;
-      const int fa = __ldg(&pr->fa), fb = __ldg(&pr->fb);
-      if (fa != cur_fa) {
-        if (cur_fa >= 0 && active) {
+  for (uint32_t u = 0;; ++u) {
+    const uint32_t sl = u % NS, round = u / NS;
+    mbar_wait(s_full + 8 * sl, round & 1);
+    const unsigned char* rec = smem_int + sl * SLOT;
+    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
+    const int fa = h0.x, fb = h0.y;
+    if (fa < 0) break;
+    const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
+    const double ABz = *reinterpret_cast<const double*>(rec + 32);
+    if (fa != cur_fa) {
+      if (cur_fa >= 0 && active) {
 #pragma unroll
-          for (int i = 0; i < NA; ++i) atomicAdd(Gc + (int64_t)(cur_fa + i) * p.ld, Ga[i]);
-        }
-        cur_fa = fa;
-#pragma unroll
-        for (int i = 0; i < NA; ++i) { Fa[i] = Fc[(int64_t)(fa + i) * p.ld]; Ga[i] = 0.0; }
+        for (int i = 0; i < NA; ++i) atomicAdd(Gc + (int64_t)(cur_fa + i) * p.ld, Ga[i]);
       }
-      double Fb[NB], Gb[NB];
+      cur_fa = fa;
 #pragma unroll
-      for (int k = 0; k < NB; ++k) { Fb[k] = Fc[(int64_t)(fb + k) * p.ld]; Gb[k] = 0.0; }
-
-      double acc[nlev(LA, L)];
-      theta_contracted<LA, LB>(p.prims + __ldg(&pr->prim_off), __ldg(&pr->nprim), gx, gy, gz, p.boys, acc);
-      ContractSink<LA, LB> sink{Fa, Fb, Ga, Gb};
-      HrrNode<LA, LB, 0, 0, 0, L>::run(acc, __ldg(&pr->ABx), __ldg(&pr->ABy), __ldg(&pr->ABz), sink);
-
-      if (fa != fb && active) {      // a == b (same shell): one direction only
+      for (int i = 0; i < NA; ++i) { Fa[i] = Fc[(int64_t)(fa + i) * p.ld]; Ga[i] = 0.0; }
+    }
+    double Fb[NB], Gb[NB];
+    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes) + t;
 #pragma unroll
-        for (int k = 0; k < NB; ++k) atomicAdd(Gc + (int64_t)(fb + k) * p.ld, Gb[k]);
-      }
+    for (int k = 0; k < NB; ++k) { Fb[k] = Fs[k * kTile]; Gb[k] = 0.0; }
+
+    double acc[nlev(LA, L)];
+    theta_contracted<LA, LB>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
+    ContractSink<LA, LB> sink{Fa, Fb, Ga, Gb};
+    HrrNode<LA, LB, 0, 0, 0, L>::run(acc, ab0.x, ab0.y, ABz, sink);
+
+    __syncwarp();
+    if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
+    if (fa != fb && active) {                                      // a == b (same shell): one direction only
+#pragma unroll
+      for (int k = 0; k < NB; ++k) atomicAdd(Gc + (int64_t)(fb + k) * p.ld, Gb[k]);
     }
   }
   if (cur_fa >= 0 && active) {
@@ -87,7 +195,16 @@ __global__ void __launch_bounds__(128) k_debug_A(const PrimPair* prims, int npri
 
 template <int LA, int LB>
 cudaError_t launch_class(const IntParams& p, cudaStream_t s) {
-  if (p.ntiles > 0 && p.pend > p.pbeg) k_integrals<LA, LB><<<p.ntiles, kTile, 0, s>>>(p);
+  if (p.ntiles > 0 && p.pend > p.pbeg) {
+    constexpr int smem = int_smem_bytes(LA, LB);
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(k_integrals<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    k_integrals<LA, LB><<<p.ntiles, kIntThreads, smem, s>>>(p);
+  }
   return cudaGetLastError();
 }
 template <int LA, int LB>

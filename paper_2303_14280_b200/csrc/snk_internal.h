@@ -18,15 +18,33 @@ inline int class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }   // (0,0
 
 struct PrimPair;   // snk_os.cuh
 
-// One significant shell pair, oriented so that l_a >= l_b (R6); a carries the VRR, the HRR shifts to b.
-struct __align__(16) PairRec {
+// ---- pair units ------------------------------------------------------------------------------------------------
+// The significant shell pairs are streamed through shared memory (one bulk copy per unit) by the integral kernel.
+// A "unit" is one shell pair (oriented so that l_a >= l_b, R6: a carries the VRR, the HRR shifts to b) with at most
+// kUnitPrims of its primitive pairs; a pair with more primitive pairs is split into consecutive units.  Because the
+// HRR (A2) and the F-contraction (Eq. 38) are linear in the contracted Theta (R4), the units of one pair simply add.
+// Units are sorted by (class, a, b); V_j holds one bit per unit (all units of a pair share the pair's decision).
+constexpr int kUnitPrims = 8;
+struct __align__(16) UnitHdr {
   int32_t fa, fb;         // first basis-function index of shell a / b
-  int32_t prim_off;       // first PrimPair
-  int32_t nprim;          // primitive pairs kept (R14)
+  int32_t nprim;          // primitive pairs in this unit (R14 may leave 0: such a unit is never in V_j)
+  int32_t first;          // 1 for the first unit of its pair
   double ABx, ABy, ABz;   // A - B
   int32_t sa, sb;         // shell ids
+  double At;              // R11 bound of the pair
+  int32_t pad[2];
 };
-static_assert(sizeof(PairRec) == 48, "PairRec layout");
+static_assert(sizeof(UnitHdr) == 64, "UnitHdr layout");
+constexpr int kPrimBytes = 80;                                   // sizeof(PrimPair), snk_os.cuh
+constexpr int kUnitBytes = 64 + kUnitPrims * kPrimBytes;         // 704: header + primitive pairs, contiguous in HBM
+// what the screening kernels and the kernel's producer warp need, without touching the 704-byte records
+struct __align__(8) UnitMeta {
+  int32_t sa, sb;
+  int32_t fb;
+  int32_t nprim_first;    // nprim | first << 8
+  double At;
+};
+static_assert(sizeof(UnitMeta) == 24, "UnitMeta layout");
 
 // One tile = up to kTile consecutive slots of one batch.
 struct TileRec { int32_t batch; int32_t n; int64_t slot; };
@@ -66,10 +84,10 @@ struct IntParams {
   int64_t slot0;           // first slot of the super-batch
   const TileRec* tiles; int ntiles;
   const uint32_t* vmask; int64_t vstride;   // words per batch
-  int pbeg, pend;          // range of this class in the significant-pair list
-  const PairRec* pairs;
-  const PrimPair* prims;
-  const double* boys;
+  int pbeg, pend;          // range of this class in the unit list
+  const unsigned char* units;               // [nunit][kUnitBytes]
+  const UnitMeta* meta;                     // [nunit]
+  const double* boys;                       // Boys tables, all L (snk_os.cuh)
 };
 
 // ---- kernel launchers (each returns cudaGetLastError()) ----

@@ -300,53 +300,44 @@ __device__ __forceinline__ bool cand_decode(const PairCand& pc, int64_t i, int& 
   return true;
 }
 
-// candidate pair i is globally significant iff its Eq. 44/45 estimate with the per-shell maxima over batches reaches eps
+// candidate pair i is globally significant iff its Eq. 44/45 estimate with the per-shell maxima over batches reaches eps.
+// nunit[i] = number of pair units it will occupy (ceil(K_a K_b / kUnitPrims)), ispair[i] = 0/1.
 __global__ void k_pair_flags(PairCand pc, ShellTab sh, const double* __restrict__ Atil, const double* __restrict__ Fmax,
-                             const double* __restrict__ phimax, double eps, int32_t* __restrict__ flag, int32_t* __restrict__ nprim) {
+                             const double* __restrict__ phimax, double eps, int32_t* __restrict__ nunit, int32_t* __restrict__ ispair) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= pc.off[kNumClasses]) return;
-  int a, b, f = 0, np = 0;
+  int a, b, f = 0, nu = 0;
   if (cand_decode(pc, i, a, b)) {
     const double At = Atil[(int64_t)a * sh.nsh + b];
     const double fa = Fmax[a], fb = Fmax[b];
     const double eE = fa * fb * At, eK = fmax(fa, fb) * (*phimax) * At;
     f = (eE >= eps || eK >= eps) ? 1 : 0;
-    np = f ? sh.nprim[a] * sh.nprim[b] : 0;
+    nu = f ? (sh.nprim[a] * sh.nprim[b] + kUnitPrims - 1) / kUnitPrims : 0;
   }
-  flag[i] = f; nprim[i] = np;
+  nunit[i] = nu; ispair[i] = f;
 }
 
-__global__ void k_pair_compact(PairCand pc, ShellTab sh, const int32_t* __restrict__ flag, const int32_t* __restrict__ pos,
-                               const int32_t* __restrict__ ppos, const double* __restrict__ Atil, PairRec* __restrict__ pairs,
-                               double* __restrict__ pairAt) {
+// Pair units of every significant pair: header, primitive-pair table (R1 prefactor) and the screening metadata.
+// R14: a primitive pair whose rigorous s-type bound (same construction as R11) times the largest density factor of
+// Eqs. 44/45 is below prim_thresh / (K_a K_b) is dropped (never when eps = 0).  Kept primitive pairs are packed into the
+// pair's units in order; trailing units may stay empty (nprim = 0) and are then never part of V_j.
+__global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict__ nunit, const int32_t* __restrict__ pos,
+                            const double* __restrict__ Atil, double prim_thresh, const double* __restrict__ Fmax,
+                            const double* __restrict__ phimax, unsigned char* __restrict__ units, UnitMeta* __restrict__ meta) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= pc.off[kNumClasses] || !flag[i]) return;
+  if (i >= pc.off[kNumClasses] || nunit[i] == 0) return;
   int a, b;
   cand_decode(pc, i, a, b);
-  PairRec r;
-  r.fa = sh.foff[a]; r.fb = sh.foff[b]; r.prim_off = ppos[i]; r.nprim = 0;
-  r.ABx = sh.cx[a] - sh.cx[b]; r.ABy = sh.cy[a] - sh.cy[b]; r.ABz = sh.cz[a] - sh.cz[b];
-  r.sa = a; r.sb = b;
-  pairs[pos[i]] = r;
-  pairAt[pos[i]] = Atil[(int64_t)a * sh.nsh + b];
-}
-
-// primitive-pair table of every significant pair (R1 prefactor); R14: a primitive pair whose rigorous s-type bound
-// (same construction as R11) is below prim_thresh / (K_a K_b) is dropped (never when eps = 0).
-__global__ void k_prim_fill(int npair, ShellTab sh, PairRec* __restrict__ pairs, PrimPair* __restrict__ prims, double prim_thresh,
-                            const double* __restrict__ Fmax, const double* __restrict__ phimax) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npair) return;
-  PairRec r = pairs[i];
-  const int a = r.sa, b = r.sb;
   const int la = sh.l[a], lb = sh.l[b];
   const int pa = sh.poff[a], pb = sh.poff[b], ka = sh.nprim[a], kb = sh.nprim[b];
   const double A[3] = {sh.cx[a], sh.cy[a], sh.cz[a]}, B[3] = {sh.cx[b], sh.cy[b], sh.cz[b]};
-  const double AB2 = r.ABx * r.ABx + r.ABy * r.ABy + r.ABz * r.ABz;
-  // density factor of Eqs. 44/45 with the per-shell maxima over batches: the dropped term's effect on K is bounded by bound * dens
+  const double ABx = A[0] - B[0], ABy = A[1] - B[1], ABz = A[2] - B[2];
+  const double AB2 = ABx * ABx + ABy * ABy + ABz * ABz;
+  const double At = Atil[(int64_t)a * sh.nsh + b];
   const double dens = fmax(Fmax[a] * Fmax[b], fmax(Fmax[a], Fmax[b]) * (*phimax));
   const double thr = prim_thresh / (double)(ka * kb);
-  int n = 0;
+  const int u0 = pos[i], nu = nunit[i];
+  int n = 0;                                   // primitive pairs kept so far
   for (int k = 0; k < ka; ++k)
     for (int l = 0; l < kb; ++l) {
       const double za = sh.pexp[pa + k], zb = sh.pexp[pb + l], ca = sh.pcoef[pa + k], cb = sh.pcoef[pb + l];
@@ -364,47 +355,62 @@ __global__ void k_prim_fill(int npair, ShellTab sh, PairRec* __restrict__ pairs,
       q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
       q.pref = ca * cb * (6.283185307179586 / q.p) * exp(-(za * zb / q.p) * AB2);
       q.pad = 0.0;
-      prims[r.prim_off + n] = q;
+      *reinterpret_cast<PrimPair*>(units + (size_t)(u0 + n / kUnitPrims) * kUnitBytes + 64 + (n % kUnitPrims) * kPrimBytes) = q;
       ++n;
     }
-  pairs[i].nprim = n;
+  for (int u = 0; u < nu; ++u) {
+    const int np = max(0, min(kUnitPrims, n - u * kUnitPrims));
+    UnitHdr h;
+    h.fa = sh.foff[a]; h.fb = sh.foff[b]; h.nprim = np; h.first = u == 0;
+    h.ABx = ABx; h.ABy = ABy; h.ABz = ABz; h.sa = a; h.sb = b; h.At = At; h.pad[0] = h.pad[1] = 0;
+    *reinterpret_cast<UnitHdr*>(units + (size_t)(u0 + u) * kUnitBytes) = h;
+    UnitMeta m;
+    m.sa = a; m.sb = b; m.fb = h.fb; m.nprim_first = np | ((u == 0) << 8); m.At = At;
+    meta[u0 + u] = m;
+  }
 }
 
-// V_j bit masks (Eq. 43): one thread per (batch, significant pair)
-__global__ void k_vmask(int npair, const PairRec* __restrict__ pairs, const double* __restrict__ pairAt, const double* __restrict__ FtsT,
-                        int nshld, const double* __restrict__ phit, double eps, uint32_t* __restrict__ vmask, int64_t vstride) {
+// V_j bit masks (Eq. 43): one thread per (batch, unit); every unit of a pair takes the pair's decision
+__global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const double* __restrict__ FtsT, int nshld,
+                        const double* __restrict__ phit, double eps, uint32_t* __restrict__ vmask, int64_t vstride) {
   const int j = blockIdx.y;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   bool keep = false;
-  if (i < npair) {
+  if (i < nunit) {
+    const UnitMeta m = meta[i];
     const double* F = FtsT + (int64_t)j * nshld;
-    const double fa = F[pairs[i].sa], fb = F[pairs[i].sb], At = pairAt[i];
-    const double eE = fa * fb * At, eK = fmax(fa, fb) * phit[j] * At;
-    keep = (eE >= eps || eK >= eps) && pairs[i].nprim > 0;
+    const double fa = F[m.sa], fb = F[m.sb];
+    const double eE = fa * fb * m.At, eK = fmax(fa, fb) * phit[j] * m.At;
+    keep = (eE >= eps || eK >= eps) && (m.nprim_first & 0xff) > 0;
   }
   const unsigned bal = __ballot_sync(~0u, keep);
   if ((threadIdx.x & 31) == 0 && (i >> 5) < vstride) vmask[(int64_t)j * vstride + (i >> 5)] = bal;
 }
 
 // counters for snk_stats: out[0]=sum|V_j|, [1]=pair-points, [2]=contracted integrals, [3]=primitive integrals,
-// [4..13] contracted integrals per class, [14] flop model, [16..25] flop model per class
-__global__ void k_vstats(int npair, const PairRec* __restrict__ pairs, ShellTab sh, const int32_t* __restrict__ bn,
+// [4..13] contracted integrals per class, [14] flop model, [16..25] flop model per class.  Pair-level quantities are
+// counted on the first unit of a pair only.
+__global__ void k_vstats(int nunit, const UnitMeta* __restrict__ meta, ShellTab sh, const int32_t* __restrict__ bn,
                          const uint32_t* __restrict__ vmask, int64_t vstride, const double* __restrict__ class_flops_prim,
                          const double* __restrict__ class_flops_contr, double* __restrict__ out) {
   const int j = blockIdx.y;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npair) return;
+  if (i >= nunit) return;
   if (!((vmask[(int64_t)j * vstride + (i >> 5)] >> (i & 31)) & 1u)) return;
-  const PairRec r = pairs[i];
-  const int la = sh.l[r.sa], lb = sh.l[r.sb];
+  const UnitMeta m = meta[i];
+  const int la = sh.l[m.sa], lb = sh.l[m.sb];
+  const int np = m.nprim_first & 0xff;
+  const double first = (double)((m.nprim_first >> 8) & 1);
   const double nq = bn[j], nc = (double)(ncart(la) * ncart(lb));
   const int cls = la * (la + 1) / 2 + lb;
-  atomicAdd(out + 0, 1.0);
-  atomicAdd(out + 1, nq);
-  atomicAdd(out + 2, nq * nc);
-  atomicAdd(out + 3, nq * nc * r.nprim);
-  atomicAdd(out + 4 + cls, nq * nc);
-  const double fl = nq * (class_flops_prim[cls] * r.nprim + class_flops_contr[cls]);
+  if (first > 0.0) {
+    atomicAdd(out + 0, 1.0);
+    atomicAdd(out + 1, nq);
+    atomicAdd(out + 2, nq * nc);
+    atomicAdd(out + 4 + cls, nq * nc);
+  }
+  atomicAdd(out + 3, nq * nc * np);
+  const double fl = nq * (class_flops_prim[cls] * np + class_flops_contr[cls] * first);
   atomicAdd(out + 14, fl);
   atomicAdd(out + 16 + cls, fl);
 }
@@ -547,39 +553,34 @@ cudaError_t run_shell_max(const ShellTab& sh, int nbatch, const double* Ftf, int
 }
 
 cudaError_t run_pair_flags(const PairCand& pc, const ShellTab& sh, const double* Atil, const double* Fmax, const double* phimax, double eps,
-                           int32_t* flag, int32_t* nprim, cudaStream_t s) {
+                           int32_t* nunit, int32_t* ispair, cudaStream_t s) {
   const int64_t n = pc.off[kNumClasses];
-  if (n > 0) k_pair_flags<<<nblk(n, 256), 256, 0, s>>>(pc, sh, Atil, Fmax, phimax, eps, flag, nprim);
+  if (n > 0) k_pair_flags<<<nblk(n, 256), 256, 0, s>>>(pc, sh, Atil, Fmax, phimax, eps, nunit, ispair);
   return cudaGetLastError();
 }
 
-cudaError_t run_pair_compact(const PairCand& pc, const ShellTab& sh, const int32_t* flag, const int32_t* pos, const int32_t* ppos,
-                             const double* Atil, PairRec* pairs, double* pairAt, cudaStream_t s) {
+cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t* nunit, const int32_t* pos, const double* Atil,
+                          double prim_thresh, const double* Fmax, const double* phimax, unsigned char* units, UnitMeta* meta,
+                          cudaStream_t s) {
   const int64_t n = pc.off[kNumClasses];
-  if (n > 0) k_pair_compact<<<nblk(n, 256), 256, 0, s>>>(pc, sh, flag, pos, ppos, Atil, pairs, pairAt);
+  if (n > 0) k_unit_fill<<<nblk(n, 128), 128, 0, s>>>(pc, sh, nunit, pos, Atil, prim_thresh, Fmax, phimax, units, meta);
   return cudaGetLastError();
 }
 
-cudaError_t run_prim_fill(int npair, const ShellTab& sh, PairRec* pairs, PrimPair* prims, double prim_thresh, const double* Fmax,
-                          const double* phimax, cudaStream_t s) {
-  if (npair > 0) k_prim_fill<<<nblk(npair, 128), 128, 0, s>>>(npair, sh, pairs, prims, prim_thresh, Fmax, phimax);
-  return cudaGetLastError();
-}
-
-cudaError_t run_vmask(int nbatch, int npair, const PairRec* pairs, const double* pairAt, const double* FtsT, int nshld, const double* phit,
-                      double eps, uint32_t* vmask, int64_t vstride, cudaStream_t s) {
-  if (nbatch > 0 && npair > 0) {
-    dim3 g(nblk(npair, 256), (unsigned)nbatch);
-    k_vmask<<<g, 256, 0, s>>>(npair, pairs, pairAt, FtsT, nshld, phit, eps, vmask, vstride);
+cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
+                      uint32_t* vmask, int64_t vstride, cudaStream_t s) {
+  if (nbatch > 0 && nunit > 0) {
+    dim3 g(nblk(nunit, 256), (unsigned)nbatch);
+    k_vmask<<<g, 256, 0, s>>>(nunit, meta, FtsT, nshld, phit, eps, vmask, vstride);
   }
   return cudaGetLastError();
 }
 
-cudaError_t run_vstats(int nbatch, int npair, const PairRec* pairs, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
+cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
                        int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s) {
-  if (nbatch > 0 && npair > 0) {
-    dim3 g(nblk(npair, 256), (unsigned)nbatch);
-    k_vstats<<<g, 256, 0, s>>>(npair, pairs, sh, bn, vmask, vstride, cfp, cfc, out);
+  if (nbatch > 0 && nunit > 0) {
+    dim3 g(nblk(nunit, 256), (unsigned)nbatch);
+    k_vstats<<<g, 256, 0, s>>>(nunit, meta, sh, bn, vmask, vstride, cfp, cfc, out);
   }
   return cudaGetLastError();
 }

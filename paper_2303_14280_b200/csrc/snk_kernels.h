@@ -36,14 +36,13 @@ cudaError_t run_abs(int64_t n, const double* in, double* out, cudaStream_t s);
 cudaError_t run_shell_max(const ShellTab& sh, int nbatch, const double* Ftf, int64_t ldj, double* FtsT, int nshld,
                           unsigned long long* Fmax_bits, cudaStream_t s);
 cudaError_t run_pair_flags(const PairCand& pc, const ShellTab& sh, const double* Atil, const double* Fmax, const double* phimax, double eps,
-                           int32_t* flag, int32_t* nprim, cudaStream_t s);
-cudaError_t run_pair_compact(const PairCand& pc, const ShellTab& sh, const int32_t* flag, const int32_t* pos, const int32_t* ppos,
-                             const double* Atil, PairRec* pairs, double* pairAt, cudaStream_t s);
-cudaError_t run_prim_fill(int npair, const ShellTab& sh, PairRec* pairs, PrimPair* prims, double prim_thresh, const double* Fmax,
-                          const double* phimax, cudaStream_t s);
-cudaError_t run_vmask(int nbatch, int npair, const PairRec* pairs, const double* pairAt, const double* FtsT, int nshld, const double* phit,
-                      double eps, uint32_t* vmask, int64_t vstride, cudaStream_t s);
-cudaError_t run_vstats(int nbatch, int npair, const PairRec* pairs, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
+                           int32_t* nunit, int32_t* ispair, cudaStream_t s);
+cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t* nunit, const int32_t* pos, const double* Atil,
+                          double prim_thresh, const double* Fmax, const double* phimax, unsigned char* units, UnitMeta* meta,
+                          cudaStream_t s);
+cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
+                      uint32_t* vmask, int64_t vstride, cudaStream_t s);
+cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
                        int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s);
 cudaError_t run_colloc(const ShellTab& sh, const TileRec* tiles, int ntiles, const double* gx, const double* gy, const double* gz,
                        const uint32_t* bmask, int nshw, double* Phi, int64_t ld, int64_t slot0, cudaStream_t s);

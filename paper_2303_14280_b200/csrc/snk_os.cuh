@@ -46,41 +46,51 @@ __device__ __forceinline__ void static_for(F&& f) {
 
 // ------------------------------------------------------------------------------------------------
 // Boys function, Eq. 22, reading R15:
-//   x < xmax(L): 8-term Taylor about the nearest node of a Delta = 1/16 table of F_m(x_i) at the top
-//                order m = L (dF_m/dx = -F_{m+1}), then downward recursion
-//                F_{m-1} = (2x F_m + e^{-x})/(2m-1)
+//   x < xmax(L): 8-term Taylor about the nearest node x_i of a Delta = 1/16 grid at the top order m = L
+//                (dF_m/dx = -F_{m+1}):  F_L(x) = sum_k [F_{L+k}(x_i)/k!] d^k,  d = x_i - x, |d| <= 1/32,
+//                then downward recursion F_{m-1} = (2x F_m + e^{-x})/(2m-1) with
+//                e^{-x} = e^{-x_i} e^{d}, e^{d} by its 8-term Taylor series (remainder < 3e-17).
 //   x >= xmax(L): F_0 = sqrt(pi/x)/2 and upward F_{m+1} = (2m+1) F_m / (2x); the neglected e^{-x}
 //                terms are < 4e-16 relative at xmax(L).
-// Table layout: tab[i*kBoysStride + m], m = 0..kBoysOrders-1, built on the host in snk_api.cu.
+// Table layout (built on the host in snk_api.cu): one table per top order L = 0..kBoysLmax,
+//   tab[(L*kBoysRows + i)*kBoysStride + k] = F_{L+k}(x_i)/k!  (k = 0..7),  [8] = e^{-x_i},  [9] = 0,
+// so one evaluation is four (L = 0) or five 16-byte loads from an L1-resident 53-66 KB table.
 // ------------------------------------------------------------------------------------------------
-constexpr int kBoysStride = 16;
-constexpr int kBoysOrders = 14;            // up to L + 7 with L = 6
+constexpr int kBoysStride = 10;
+constexpr int kBoysLmax = 6;
 constexpr double kBoysDelta = 1.0 / 16.0;
 constexpr int kBoysRows = 52 * 16 + 2;
 __host__ __device__ constexpr double boys_xmax(int L) {
   return L == 0 ? 34.0 : L == 1 ? 38.0 : L == 2 ? 40.0 : L == 3 ? 44.0 : L == 4 ? 46.0 : L == 5 ? 50.0 : 52.0;
 }
 
+// tab = base of the whole table set
 template <int L>
 __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
   if (x < boys_xmax(L)) {
     const int i = __double2int_rn(x * 16.0);
-    const double d = (double)i * kBoysDelta - x;     // F_m(x) = sum_k F_{m+k}(x_i) d^k / k!
-    const double* row = tab + i * kBoysStride + L;
-    double t[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) t[k] = __ldg(row + k);
-    double s = t[7] * (1.0 / 7.0);
-    s = fma(s, d, t[6]) * (1.0 / 6.0);
-    s = fma(s, d, t[5]) * (1.0 / 5.0);
-    s = fma(s, d, t[4]) * (1.0 / 4.0);
-    s = fma(s, d, t[3]) * (1.0 / 3.0);
-    s = fma(s, d, t[2]) * 0.5;
-    s = fma(s, d, t[1]);
-    F[L] = fma(s, d, t[0]);
+    const double d = fma((double)i, kBoysDelta, -x);
+    const double2* __restrict__ row = reinterpret_cast<const double2*>(tab + ((size_t)L * kBoysRows + i) * kBoysStride);
+    const double2 t01 = __ldg(row), t23 = __ldg(row + 1), t45 = __ldg(row + 2), t67 = __ldg(row + 3);
+    double s = fma(t67.y, d, t67.x);
+    s = fma(s, d, t45.y);
+    s = fma(s, d, t45.x);
+    s = fma(s, d, t23.y);
+    s = fma(s, d, t23.x);
+    s = fma(s, d, t01.y);
+    F[L] = fma(s, d, t01.x);
     if constexpr (L > 0) {
-      const double ex = exp(-x);
-      const double x2 = 2.0 * x;
+      const double2 e = __ldg(row + 4);
+      double q = 1.0 / 5040.0;
+      q = fma(q, d, 1.0 / 720.0);
+      q = fma(q, d, 1.0 / 120.0);
+      q = fma(q, d, 1.0 / 24.0);
+      q = fma(q, d, 1.0 / 6.0);
+      q = fma(q, d, 0.5);
+      q = fma(q, d, 1.0);
+      q = fma(q, d, 1.0);
+      const double ex = e.x * q;
+      const double x2 = x + x;
 #pragma unroll
       for (int m = L; m >= 1; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
     }
@@ -218,7 +228,8 @@ struct StoreSink {
   }
 };
 
-// Contracted Theta^0 (levels LA..LA+LB) of one shell pair at one point.
+// Contracted Theta^0 (levels LA..LA+LB) of one shell pair (unit) at one point.  pp points at the unit's primitive
+// pairs: shared memory in the build kernel (every lane reads the same address: broadcast), global in the test hook.
 template <int LA, int LB>
 __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp, int nprim, double gx, double gy, double gz,
                                                  const double* __restrict__ boys_tab, double (&acc)[nlev(LA, LA + LB)]) {
@@ -226,18 +237,20 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
 #pragma unroll
   for (int i = 0; i < nlev(LA, L); ++i) acc[i] = 0.0;
   for (int k = 0; k < nprim; ++k) {
-    const double p = __ldg(&pp[k].p);
-    const double PCx = __ldg(&pp[k].Px) - gx, PCy = __ldg(&pp[k].Py) - gy, PCz = __ldg(&pp[k].Pz) - gz;
-    const double x = p * fma(PCx, PCx, fma(PCy, PCy, PCz * PCz));
+    const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k);
+    const double2 q0 = q[0], q1 = q[1], q2 = q[2];   // (p, inv2p) (Px, Py) (Pz, PAx)
+    const double PCx = q1.x - gx, PCy = q1.y - gy, PCz = q2.x - gz;
+    const double x = q0.x * fma(PCx, PCx, fma(PCy, PCy, PCz * PCz));
     double th0[L + 1];
     boys<L>(x, boys_tab, th0);
-    const double pref = __ldg(&pp[k].pref);
-#pragma unroll
-    for (int n = 0; n <= L; ++n) th0[n] *= pref;
+    const double2 q4 = q[4];                          // (pref, pad)
     if constexpr (L == 0) {
-      acc[0] += th0[0];
+      acc[0] = fma(th0[0], q4.x, acc[0]);
     } else {
-      vrr_accumulate<LA, L>(th0, __ldg(&pp[k].PAx), __ldg(&pp[k].PAy), __ldg(&pp[k].PAz), PCx, PCy, PCz, __ldg(&pp[k].inv2p), acc);
+      const double2 q3 = q[3];                        // (PAy, PAz)
+#pragma unroll
+      for (int n = 0; n <= L; ++n) th0[n] *= q4.x;
+      vrr_accumulate<LA, L>(th0, q2.y, q3.x, q3.y, PCx, PCy, PCz, q0.y, acc);
     }
   }
 }
