@@ -21,7 +21,7 @@ namespace snk {
 constexpr int kConsumerWarps = kTile / 32;
 constexpr int kIntThreads = kTile + 32;
 
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : (LA + LB >= 2 ? 6 : 8); }
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : (LA + LB >= 2 ? 8 : 16); }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
 __host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB); }
 
@@ -48,6 +48,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
+// producer-side wait: poll with back-off so that the waiting lane does not steal issue slots from the consumer warps
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  for (;;) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (done) break;
+    __nanosleep(200);
+  }
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
                "r"(bar)
@@ -57,7 +74,7 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 template <int LA, int LB>
 __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
-  constexpr int NS = int_nslots(LA, LB), SLOT = int_slot_bytes(LB);
+  constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
   extern __shared__ __align__(128) unsigned char smem_int[];
   const uint32_t s_base = smem_u32(smem_int);
   const uint32_t s_full = s_base + NS * SLOT, s_empty = s_full + NS * 8;
@@ -91,14 +108,20 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
         const uint32_t bits = __shfl_sync(~0u, word, src);
         const int n = __popc(bits);
         const int base_pid = (wb + src) << 5;
-        for (int b0 = 0; b0 < n; b0 += NS) {               // at most NS units in flight per step: one lane per unit
-          const bool mine = lane >= b0 && lane < min(n, b0 + NS);
+        for (int b0 = 0; b0 < n; b0 += NG) {               // NG units per step (half the ring): one lane per unit
+          const int cnt = min(n, b0 + NG) - b0;
+          const bool mine = lane >= b0 && lane < b0 + cnt;
+          int pid = 0;
+          UnitMeta m{};
+          if (mine) { pid = base_pid + (int)__fns(bits, 0, lane + 1); m = p.meta[pid]; }   // in flight while we wait for slots
+          // slots are released in unit order, so the step's last slot being free implies the others are: one lane polls
+          if (lane == 0) {
+            const uint32_t last = u + (uint32_t)cnt - 1u;
+            if (last >= NS) mbar_wait_backoff(s_empty + 8 * (last % NS), (last / NS - 1) & 1);
+          }
+          __syncwarp();
           if (mine) {
-            const int pid = base_pid + (int)__fns(bits, 0, lane + 1);
-            const UnitMeta m = p.meta[pid];
-            const uint32_t uu = u + (uint32_t)(lane - b0);
-            const uint32_t slot = uu % NS, round = uu / NS;
-            if (round > 0) mbar_wait(s_empty + 8 * slot, (round - 1) & 1);
+            const uint32_t slot = (u + (uint32_t)(lane - b0)) % NS;
             const uint32_t nb = 64u + (uint32_t)(m.nprim_first & 0xff) * (uint32_t)kPrimBytes;
             const uint32_t bar = s_full + 8 * slot, dst = s_base + slot * SLOT;
             mbar_arrive_expect_tx(bar, nb + NB * frow);
@@ -107,14 +130,14 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
 #pragma unroll
             for (int k = 0; k < NB; ++k) bulk_g2s(dst + kUnitBytes + k * (kTile * 8), Fsrc + (int64_t)k * p.ld, frow, bar);
           }
-          u += (uint32_t)(min(n, b0 + NS) - b0);
+          u += (uint32_t)cnt;
           __syncwarp();
         }
       }
     }
     if (lane == 0) {                                       // end-of-list sentinel: a header with fa = -1
       const uint32_t slot = u % NS, round = u / NS;
-      if (round > 0) mbar_wait(s_empty + 8 * slot, (round - 1) & 1);
+      if (round > 0) mbar_wait_backoff(s_empty + 8 * slot, (round - 1) & 1);
       reinterpret_cast<volatile int32_t*>(smem_int + slot * SLOT)[0] = -1;
       mbar_arrive(s_full + 8 * slot);
     }
@@ -134,9 +157,9 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
 #pragma unroll
   for (int i = 0; i < NA; ++i) { Fa[i] = 0.0; Ga[i] = 0.0; }
 
-  for (uint32_t u = 0;; ++u) {
-    const uint32_t sl = u % NS, round = u / NS;
-    mbar_wait(s_full + 8 * sl, round & 1);
+  uint32_t sl = 0, phase = 0;
+  for (;;) {
+    mbar_wait(s_full + 8 * sl, phase);
     const unsigned char* rec = smem_int + sl * SLOT;
     const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
     const int fa = h0.x, fb = h0.y;
@@ -164,6 +187,7 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
 
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
+    if (++sl == NS) { sl = 0; phase ^= 1; }
     if (fa != fb && active) {                                      // a == b (same shell): one direction only
 #pragma unroll
       for (int k = 0; k < NB; ++k) atomicAdd(Gc + (int64_t)(fb + k) * p.ld, Gb[k]);

@@ -68,8 +68,11 @@ __host__ __device__ constexpr double boys_xmax(int L) {
 template <int L>
 __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
   if (x < boys_xmax(L)) {
-    const int i = __double2int_rn(x * 16.0);
-    const double d = fma((double)i, kBoysDelta, -x);
+    // nearest node without F2I/I2F (the conversion pipe is 4x slower than the FP64 pipe): adding 1.5*2^52 leaves
+    // round-to-nearest(16 x) in the low mantissa bits
+    const double tm = fma(x, 16.0, 6755399441055744.0);
+    const int i = __double2loint(tm);
+    const double d = fma(tm - 6755399441055744.0, kBoysDelta, -x);
     const double2* __restrict__ row = reinterpret_cast<const double2*>(tab + ((size_t)L * kBoysRows + i) * kBoysStride);
     const double2 t01 = __ldg(row), t23 = __ldg(row + 1), t45 = __ldg(row + 2), t67 = __ldg(row + 3);
     double s = fma(t67.y, d, t67.x);
@@ -95,7 +98,11 @@ __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, d
       for (int m = L; m >= 1; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
     }
   } else {
-    const double r = rsqrt(x);
+    // 1/sqrt(x) for 34 <= x < inf: hardware seed (2^-22) + one third-order step; no special cases can occur here
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    const double e = fma(-x, y0 * y0, 1.0);
+    const double r = fma(fma(e, 0.375, 0.5), y0 * e, y0);
     F[0] = 0.88622692545275801365 * r;               // sqrt(pi)/2
     if constexpr (L > 0) {
       const double h = 0.5 * r * r;                  // 1/(2x)
