@@ -133,6 +133,21 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def _ncu_traffic(cfg, cls_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+    summary of this same workload (profiles/ncu_full_cfg<cfg>.csv); None when no capture of it is committed."""
+    path = os.path.join(ROOT, "profiles", "ncu_full_cfg%d.csv" % cfg)
+    try:
+        import csv
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["class"] == cls_name:
+                    return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
+    except Exception:
+        pass
+    return None
+
+
 def _gen_device():
     try:
         import torch
@@ -213,6 +228,7 @@ def main():
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.cudart().cudaProfilerStart()      # `ncu --profile-from-start off` then sees exactly the timed region
     t0 = time.time()
     e0.record()
     for _ in range(args.steps):
@@ -220,6 +236,7 @@ def main():
     e1.record()
     barrier()
     t1 = time.time()
+    torch.cuda.cudart().cudaProfilerStop()
     ms = e0.elapsed_time(e1)
     st = s.stats()            # per-stage CUDA-event times of the LAST timed step (recorded inside the timed region)
     clocks = sampler.stop(t0, t1) if sampler else None
@@ -265,7 +282,7 @@ def main():
     achieved = k_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
     all_ms = sum(st["ms_G_class"])
     roofline = {"bound": "alu", "kernel": "k_integrals<%s>" % snk.CLASS_NAMES[cls], "achieved": achieved, "peak": dfma_peak, "unit": "TFLOP/s",
-                "frac": achieved / dfma_peak if dfma_peak else None, "traffic": None,
+                "frac": achieved / dfma_peak if dfma_peak else None, "traffic": _ncu_traffic(args.config, snk.CLASS_NAMES[cls]),
                 "peak_source": "measured on this GPU by snk_measure_fp64_peak (register-resident DFMA loop); nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2",
                 "flops_per_launch": k_flops, "ms_per_launch": k_ms,
                 "all_integral_kernels": {"achieved": st["flops_integral"] / (all_ms * 1e-3) * 1e-12 if all_ms > 0 else 0.0, "ms": all_ms,

@@ -18,10 +18,16 @@
 
 namespace snk {
 
-constexpr int kConsumerWarps = kTile / 32;
-constexpr int kIntThreads = kTile + 32;
+// points per consumer thread: two for the low-L classes (their registers allow it), one otherwise
+__host__ __device__ constexpr int int_npmax(int LA, int LB) { return 1; }
+// resident CTAs per SM the register allocation is held to (the kernel is latency bound: warps in flight matter most)
+__host__ __device__ constexpr int int_minblocks(int LA, int LB) {
+  const int L = LA + LB;
+  return L == 0 ? 7 : L == 1 ? 4 : L == 2 ? 4 : L == 3 ? 3 : L == 4 ? 2 : 1;
+}
+__host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile / int_npmax(LA, LB) + 32; }
 
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : (LA + LB >= 2 ? 8 : 16); }
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : 8; }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
 __host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB); }
 
@@ -71,9 +77,101 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                : "memory");
 }
 
-template <int LA, int LB>
-__global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
+// ---- consumer side: the whole unit stream for the 32*NP points [pbase, pbase + 32 NP) of the tile, NP points per thread ----
+template <int LA, int LB, int NP>
+__device__ __forceinline__ void consume_units(const IntParams& p, const unsigned char* smem_int, uint32_t s_full, uint32_t s_empty,
+                                              const TileRec& tile, int64_t col0, int pbase, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
+  constexpr int NS = int_nslots(LA, LB), SLOT = int_slot_bytes(LB);
+  int pt[NP], ptc[NP];
+  bool act[NP];
+  double gx[NP], gy[NP], gz[NP];
+#pragma unroll
+  for (int s = 0; s < NP; ++s) {
+    pt[s] = pbase + 32 * s + lane;
+    act[s] = pt[s] < tile.n;
+    ptc[s] = act[s] ? pt[s] : tile.n - 1;             // inactive lanes shadow the tile's last point and never write
+    const int64_t slot = tile.slot + ptc[s];
+    gx[s] = p.gx[slot]; gy[s] = p.gy[slot]; gz[s] = p.gz[slot];
+  }
+  const double* __restrict__ Fc[NP];
+  double* __restrict__ Gc[NP];
+#pragma unroll
+  for (int s = 0; s < NP; ++s) { Fc[s] = p.F + col0 + ptc[s]; Gc[s] = p.G + col0 + pt[s]; }
+  const int64_t ld = p.ld;
+
+  int cur_fa = -1;
+  double Fa[NP][NA], Ga[NP][NA];
+#pragma unroll
+  for (int s = 0; s < NP; ++s)
+#pragma unroll
+    for (int i = 0; i < NA; ++i) { Fa[s][i] = 0.0; Ga[s][i] = 0.0; }
+
+  uint32_t sl = 0, phase = 0;
+  for (;;) {
+    mbar_wait(s_full + 8 * sl, phase);
+    const unsigned char* rec = smem_int + sl * SLOT;
+    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
+    const int fa = h0.x, fb = h0.y;
+    if (fa < 0) break;
+    const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
+    const double ABz = *reinterpret_cast<const double*>(rec + 32);
+    if (fa != cur_fa) {
+      if (cur_fa >= 0) {
+#pragma unroll
+        for (int s = 0; s < NP; ++s)
+          if (act[s]) {
+#pragma unroll
+            for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + (int64_t)(cur_fa + i) * ld, Ga[s][i]);
+          }
+      }
+      cur_fa = fa;
+#pragma unroll
+      for (int s = 0; s < NP; ++s)
+#pragma unroll
+        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[s][(int64_t)(fa + i) * ld]; Ga[s][i] = 0.0; }
+    }
+    double Fb[NP][NB], Gb[NP][NB];
+    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+#pragma unroll
+      for (int k = 0; k < NB; ++k) { Fb[s][k] = Fs[k * kTile + ptc[s]]; Gb[s][k] = 0.0; }
+
+    double acc[NP][nlev(LA, L)];
+    theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
+#pragma unroll
+    for (int s = 0; s < NP; ++s) {
+      ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
+      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ab0.x, ab0.y, ABz, sink);
+    }
+
+    __syncwarp();
+    if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
+    if (++sl == NS) { sl = 0; phase ^= 1; }
+    if (fa != fb) {                                                // a == b (same shell): one direction only
+#pragma unroll
+      for (int s = 0; s < NP; ++s)
+        if (act[s]) {
+#pragma unroll
+          for (int k = 0; k < NB; ++k) atomicAdd(Gc[s] + (int64_t)(fb + k) * ld, Gb[s][k]);
+        }
+    }
+  }
+  if (cur_fa >= 0) {
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+      if (act[s]) {
+#pragma unroll
+        for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + (int64_t)(cur_fa + i) * ld, Ga[s][i]);
+      }
+  }
+}
+
+template <int LA, int LB>
+__global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_integrals(IntParams p) {
+  constexpr int NB = ncart(LB);
+  constexpr int NPM = int_npmax(LA, LB), CW = kTile / (32 * NPM);   // points per thread, consumer warps per CTA
   constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
   extern __shared__ __align__(128) unsigned char smem_int[];
   const uint32_t s_base = smem_u32(smem_int);
@@ -81,8 +179,8 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
 
   const TileRec tile = p.tiles[blockIdx.x];
   const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-  const int nw = (tile.n + 31) >> 5;                       // consumer warps that own at least one point
-  const int npad = nw << 5;
+  const int nw = (tile.n + 32 * NPM - 1) / (32 * NPM);     // consumer warps that own at least one point
+  const int npad = ((tile.n + 31) >> 5) << 5;
   if (t == 0) {
     for (int i = 0; i < NS; ++i) { mbar_init(s_full + 8 * i, 1); mbar_init(s_empty + 8 * i, nw); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -90,7 +188,7 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
   __syncthreads();
   const int64_t col0 = tile.slot - p.slot0;
 
-  if (warp == kConsumerWarps) {
+  if (warp == CW) {
     // ------------------------------------------------ producer warp ------------------------------------------------
     const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
     const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
@@ -144,58 +242,12 @@ __global__ void __launch_bounds__(kIntThreads) k_integrals(IntParams p) {
     return;
   }
   if (warp >= nw) return;
-
-  // -------------------------------------------------- consumer warps --------------------------------------------------
-  const bool active = t < tile.n;
-  const int64_t slot = tile.slot + (active ? t : tile.n - 1);
-  const double gx = p.gx[slot], gy = p.gy[slot], gz = p.gz[slot];
-  const double* __restrict__ Fc = p.F + col0 + t;
-  double* __restrict__ Gc = p.G + col0 + t;
-
-  int cur_fa = -1;
-  double Fa[NA], Ga[NA];
-#pragma unroll
-  for (int i = 0; i < NA; ++i) { Fa[i] = 0.0; Ga[i] = 0.0; }
-
-  uint32_t sl = 0, phase = 0;
-  for (;;) {
-    mbar_wait(s_full + 8 * sl, phase);
-    const unsigned char* rec = smem_int + sl * SLOT;
-    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
-    const int fa = h0.x, fb = h0.y;
-    if (fa < 0) break;
-    const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
-    const double ABz = *reinterpret_cast<const double*>(rec + 32);
-    if (fa != cur_fa) {
-      if (cur_fa >= 0 && active) {
-#pragma unroll
-        for (int i = 0; i < NA; ++i) atomicAdd(Gc + (int64_t)(cur_fa + i) * p.ld, Ga[i]);
-      }
-      cur_fa = fa;
-#pragma unroll
-      for (int i = 0; i < NA; ++i) { Fa[i] = Fc[(int64_t)(fa + i) * p.ld]; Ga[i] = 0.0; }
-    }
-    double Fb[NB], Gb[NB];
-    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes) + t;
-#pragma unroll
-    for (int k = 0; k < NB; ++k) { Fb[k] = Fs[k * kTile]; Gb[k] = 0.0; }
-
-    double acc[nlev(LA, L)];
-    theta_contracted<LA, LB>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
-    ContractSink<LA, LB> sink{Fa, Fb, Ga, Gb};
-    HrrNode<LA, LB, 0, 0, 0, L>::run(acc, ab0.x, ab0.y, ABz, sink);
-
-    __syncwarp();
-    if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
-    if (++sl == NS) { sl = 0; phase ^= 1; }
-    if (fa != fb && active) {                                      // a == b (same shell): one direction only
-#pragma unroll
-      for (int k = 0; k < NB; ++k) atomicAdd(Gc + (int64_t)(fb + k) * p.ld, Gb[k]);
-    }
-  }
-  if (cur_fa >= 0 && active) {
-#pragma unroll
-    for (int i = 0; i < NA; ++i) atomicAdd(Gc + (int64_t)(cur_fa + i) * p.ld, Ga[i]);
+  const int pbase = warp * 32 * NPM;
+  if constexpr (NPM == 2) {
+    if (tile.n - pbase <= 32) consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);   // ragged tail: one point per thread
+    else consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);
+  } else {
+    consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);
   }
 }
 
@@ -205,8 +257,10 @@ __global__ void __launch_bounds__(128) k_debug_A(const PrimPair* prims, int npri
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
   const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
-  double acc[nlev(LA, L)];
-  theta_contracted<LA, LB>(prims, nprim, pts[3 * g], pts[3 * g + 1], pts[3 * g + 2], boys_tab, acc);
+  const double gx[1] = {pts[3 * g]}, gy[1] = {pts[3 * g + 1]}, gz[1] = {pts[3 * g + 2]};
+  double acc1[1][nlev(LA, L)];
+  theta_contracted<LA, LB, 1, false>(prims, nprim, gx, gy, gz, boys_tab, acc1);
+  double (&acc)[nlev(LA, L)] = acc1[0];
   double blk[NA * NB];
   StoreSink<LA, LB> sink{blk};
   HrrNode<LA, LB, 0, 0, 0, L>::run(acc, ABx, ABy, ABz, sink);
@@ -227,7 +281,7 @@ cudaError_t launch_class(const IntParams& p, cudaStream_t s) {
       if (e != cudaSuccess) return e;
       attr_set = true;
     }
-    k_integrals<LA, LB><<<p.ntiles, kIntThreads, smem, s>>>(p);
+    k_integrals<LA, LB><<<p.ntiles, int_threads(LA, LB), smem, s>>>(p);
   }
   return cudaGetLastError();
 }

@@ -64,52 +64,61 @@ __host__ __device__ constexpr double boys_xmax(int L) {
   return L == 0 ? 34.0 : L == 1 ? 38.0 : L == 2 ? 40.0 : L == 3 ? 44.0 : L == 4 ? 46.0 : L == 5 ? 50.0 : 52.0;
 }
 
-// tab = base of the whole table set
+// far field, x >= xmax(L)
+template <int L>
+__device__ __forceinline__ void boys_far(double x, double (&F)[L + 1]) {
+  // 1/sqrt(x) for 34 <= x < inf: hardware seed (2^-22) + one third-order step; no special cases can occur here
+  double y0;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+  const double e = fma(-x, y0 * y0, 1.0);
+  const double r = fma(fma(e, 0.375, 0.5), y0 * e, y0);
+  F[0] = 0.88622692545275801365 * r;               // sqrt(pi)/2
+  if constexpr (L > 0) {
+    const double h = 0.5 * r * r;                  // 1/(2x)
+#pragma unroll
+    for (int m = 0; m < L; ++m) F[m + 1] = (2 * m + 1) * F[m] * h;
+  }
+}
+
+// near field, x < xmax(L); tab = base of the whole table set
+template <int L>
+__device__ __forceinline__ void boys_near(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
+  // nearest node without F2I/I2F (the conversion pipe is 4x slower than the FP64 pipe): adding 1.5*2^52 leaves
+  // round-to-nearest(16 x) in the low mantissa bits
+  const double tm = fma(x, 16.0, 6755399441055744.0);
+  const int i = __double2loint(tm);
+  const double d = fma(tm - 6755399441055744.0, kBoysDelta, -x);
+  const double2* __restrict__ row = reinterpret_cast<const double2*>(tab + ((size_t)L * kBoysRows + i) * kBoysStride);
+  const double2 t01 = __ldg(row), t23 = __ldg(row + 1), t45 = __ldg(row + 2), t67 = __ldg(row + 3);
+  double s = fma(t67.y, d, t67.x);
+  s = fma(s, d, t45.y);
+  s = fma(s, d, t45.x);
+  s = fma(s, d, t23.y);
+  s = fma(s, d, t23.x);
+  s = fma(s, d, t01.y);
+  F[L] = fma(s, d, t01.x);
+  if constexpr (L > 0) {
+    const double2 e = __ldg(row + 4);
+    double q = 1.0 / 5040.0;
+    q = fma(q, d, 1.0 / 720.0);
+    q = fma(q, d, 1.0 / 120.0);
+    q = fma(q, d, 1.0 / 24.0);
+    q = fma(q, d, 1.0 / 6.0);
+    q = fma(q, d, 0.5);
+    q = fma(q, d, 1.0);
+    q = fma(q, d, 1.0);
+    const double ex = e.x * q;
+    const double x2 = x + x;
+#pragma unroll
+    for (int m = L; m >= 1; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
+  }
+}
+
+// per-lane dispatch (test hooks, divergent warps)
 template <int L>
 __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
-  if (x < boys_xmax(L)) {
-    // nearest node without F2I/I2F (the conversion pipe is 4x slower than the FP64 pipe): adding 1.5*2^52 leaves
-    // round-to-nearest(16 x) in the low mantissa bits
-    const double tm = fma(x, 16.0, 6755399441055744.0);
-    const int i = __double2loint(tm);
-    const double d = fma(tm - 6755399441055744.0, kBoysDelta, -x);
-    const double2* __restrict__ row = reinterpret_cast<const double2*>(tab + ((size_t)L * kBoysRows + i) * kBoysStride);
-    const double2 t01 = __ldg(row), t23 = __ldg(row + 1), t45 = __ldg(row + 2), t67 = __ldg(row + 3);
-    double s = fma(t67.y, d, t67.x);
-    s = fma(s, d, t45.y);
-    s = fma(s, d, t45.x);
-    s = fma(s, d, t23.y);
-    s = fma(s, d, t23.x);
-    s = fma(s, d, t01.y);
-    F[L] = fma(s, d, t01.x);
-    if constexpr (L > 0) {
-      const double2 e = __ldg(row + 4);
-      double q = 1.0 / 5040.0;
-      q = fma(q, d, 1.0 / 720.0);
-      q = fma(q, d, 1.0 / 120.0);
-      q = fma(q, d, 1.0 / 24.0);
-      q = fma(q, d, 1.0 / 6.0);
-      q = fma(q, d, 0.5);
-      q = fma(q, d, 1.0);
-      q = fma(q, d, 1.0);
-      const double ex = e.x * q;
-      const double x2 = x + x;
-#pragma unroll
-      for (int m = L; m >= 1; --m) F[m - 1] = fma(x2, F[m], ex) * (1.0 / (2 * m - 1));
-    }
-  } else {
-    // 1/sqrt(x) for 34 <= x < inf: hardware seed (2^-22) + one third-order step; no special cases can occur here
-    double y0;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-    const double e = fma(-x, y0 * y0, 1.0);
-    const double r = fma(fma(e, 0.375, 0.5), y0 * e, y0);
-    F[0] = 0.88622692545275801365 * r;               // sqrt(pi)/2
-    if constexpr (L > 0) {
-      const double h = 0.5 * r * r;                  // 1/(2x)
-#pragma unroll
-      for (int m = 0; m < L; ++m) F[m + 1] = (2 * m + 1) * F[m] * h;
-    }
-  }
+  if (x < boys_xmax(L)) boys_near<L>(x, tab, F);
+  else boys_far<L>(x, F);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -235,29 +244,112 @@ struct StoreSink {
   }
 };
 
-// Contracted Theta^0 (levels LA..LA+LB) of one shell pair (unit) at one point.  pp points at the unit's primitive
-// pairs: shared memory in the build kernel (every lane reads the same address: broadcast), global in the test hook.
-template <int LA, int LB>
-__device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp, int nprim, double gx, double gy, double gz,
-                                                 const double* __restrict__ boys_tab, double (&acc)[nlev(LA, LA + LB)]) {
+// Contracted Theta^0 (levels LA..LA+LB) of one shell pair (unit) at NP grid points held by this thread.  pp points at
+// the unit's primitive pairs: shared memory in the build kernel (every lane reads the same address: broadcast), global
+// in the test hook.  NP = 2 gives two independent recurrence streams per thread (the kernel is latency bound) and
+// halves the per-point cost of everything that does not depend on the point.
+// WARP: all 32 lanes call together; when every point of the warp is in the far field of a primitive pair (the common
+// case in the paper-shaped workloads) the Boys function runs without table loads or branches.
+template <int LA, int LB, int NP, bool WARP>
+__device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp, int nprim, const double (&gx)[NP], const double (&gy)[NP],
+                                                 const double (&gz)[NP], const double* __restrict__ boys_tab,
+                                                 double (&acc)[NP][nlev(LA, LA + LB)]) {
   constexpr int L = LA + LB;
+  // KP primitive pairs are advanced together (independent dependency chains: the FP64 pipe has an 8-cycle latency and
+  // one warp's recurrence is a serial chain); the far-field vote is taken once for the group.
+  constexpr int KP = (WARP && L <= 1) ? 2 : 1;
 #pragma unroll
-  for (int i = 0; i < nlev(LA, L); ++i) acc[i] = 0.0;
-  for (int k = 0; k < nprim; ++k) {
-    const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k);
-    const double2 q0 = q[0], q1 = q[1], q2 = q[2];   // (p, inv2p) (Px, Py) (Pz, PAx)
-    const double PCx = q1.x - gx, PCy = q1.y - gy, PCz = q2.x - gz;
-    const double x = q0.x * fma(PCx, PCx, fma(PCy, PCy, PCz * PCz));
-    double th0[L + 1];
-    boys<L>(x, boys_tab, th0);
-    const double2 q4 = q[4];                          // (pref, pad)
-    if constexpr (L == 0) {
-      acc[0] = fma(th0[0], q4.x, acc[0]);
+  for (int s = 0; s < NP; ++s)
+#pragma unroll
+    for (int i = 0; i < nlev(LA, L); ++i) acc[s][i] = 0.0;
+
+  auto step = [&](auto kpc, int k) {
+    constexpr int K = decltype(kpc)::value;
+    double2 q0[K], q1[K], q2[K];
+    double PCx[K][NP], PCy[K][NP], PCz[K][NP], x[K][NP], th0[K][NP][L + 1];
+    bool far = true;
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+      const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k + j);
+      q0[j] = q[0]; q1[j] = q[1]; q2[j] = q[2];     // (p, inv2p) (Px, Py) (Pz, PAx)
+#pragma unroll
+      for (int s = 0; s < NP; ++s) {
+        PCx[j][s] = q1[j].x - gx[s]; PCy[j][s] = q1[j].y - gy[s]; PCz[j][s] = q2[j].x - gz[s];
+        x[j][s] = q0[j].x * fma(PCx[j][s], PCx[j][s], fma(PCy[j][s], PCy[j][s], PCz[j][s] * PCz[j][s]));
+        far = far && x[j][s] >= boys_xmax(L);
+      }
+    }
+    bool allfar = false;
+    if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
+    if (allfar) {
+#pragma unroll
+      for (int j = 0; j < K; ++j)
+#pragma unroll
+        for (int s = 0; s < NP; ++s) boys_far<L>(x[j][s], th0[j][s]);
     } else {
-      const double2 q3 = q[3];                        // (PAy, PAz)
 #pragma unroll
-      for (int n = 0; n <= L; ++n) th0[n] *= q4.x;
-      vrr_accumulate<LA, L>(th0, q2.y, q3.x, q3.y, PCx, PCy, PCz, q0.y, acc);
+      for (int j = 0; j < K; ++j)
+#pragma unroll
+        for (int s = 0; s < NP; ++s) boys<L>(x[j][s], boys_tab, th0[j][s]);
+    }
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+      const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k + j);
+      const double2 q4 = q[4];                        // (pref, pad)
+      if constexpr (L == 0) {
+#pragma unroll
+        for (int s = 0; s < NP; ++s) acc[s][0] = fma(th0[j][s][0], q4.x, acc[s][0]);
+      } else {
+        const double2 q3 = q[3];                      // (PAy, PAz)
+#pragma unroll
+        for (int s = 0; s < NP; ++s) {
+#pragma unroll
+          for (int n = 0; n <= L; ++n) th0[j][s][n] *= q4.x;
+          vrr_accumulate<LA, L>(th0[j][s], q2[j].y, q3.x, q3.y, PCx[j][s], PCy[j][s], PCz[j][s], q0[j].y, acc[s]);
+        }
+      }
+    }
+  };
+  if constexpr (KP > 1) {
+    int k = 0;
+#pragma unroll 1
+    for (; k + KP <= nprim; k += KP) step(std::integral_constant<int, KP>{}, k);
+#pragma unroll 1
+    for (; k < nprim; ++k) step(std::integral_constant<int, 1>{}, k);
+  } else {
+    for (int k = 0; k < nprim; ++k) {
+      const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k);
+      const double2 q0 = q[0], q1 = q[1], q2 = q[2];   // (p, inv2p) (Px, Py) (Pz, PAx)
+      double PCx[NP], PCy[NP], PCz[NP], x[NP], th0[NP][L + 1];
+      bool far = true;
+#pragma unroll
+      for (int s = 0; s < NP; ++s) {
+        PCx[s] = q1.x - gx[s]; PCy[s] = q1.y - gy[s]; PCz[s] = q2.x - gz[s];
+        x[s] = q0.x * fma(PCx[s], PCx[s], fma(PCy[s], PCy[s], PCz[s] * PCz[s]));
+        far = far && x[s] >= boys_xmax(L);
+      }
+      bool allfar = false;
+      if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
+      if (allfar) {
+#pragma unroll
+        for (int s = 0; s < NP; ++s) boys_far<L>(x[s], th0[s]);
+      } else {
+#pragma unroll
+        for (int s = 0; s < NP; ++s) boys<L>(x[s], boys_tab, th0[s]);
+      }
+      const double2 q4 = q[4];                          // (pref, pad)
+      if constexpr (L == 0) {
+#pragma unroll
+        for (int s = 0; s < NP; ++s) acc[s][0] = fma(th0[s][0], q4.x, acc[s][0]);
+      } else {
+        const double2 q3 = q[3];                        // (PAy, PAz)
+#pragma unroll
+        for (int s = 0; s < NP; ++s) {
+#pragma unroll
+          for (int n = 0; n <= L; ++n) th0[s][n] *= q4.x;
+          vrr_accumulate<LA, L>(th0[s], q2.y, q3.x, q3.y, PCx[s], PCy[s], PCz[s], q0.y, acc[s]);
+        }
+      }
     }
   }
 }
