@@ -135,16 +135,23 @@ def run_reference(args, rank, world):
 
 def _ncu_traffic(cfg, cls_name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-    summary of this same workload (profiles/ncu_full_cfg<cfg>.csv); None when no capture of it is committed."""
-    path = os.path.join(ROOT, "profiles", "ncu_full_cfg%d.csv" % cfg)
-    try:
-        import csv
-        with open(path) as f:
-            for row in csv.DictReader(f):
-                if row["class"] == cls_name:
-                    return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
-    except Exception:
-        pass
+    summary of this same workload (newest profiles/*_ncu_full_cfg<cfg>.csv); None when no capture of it is committed."""
+    import csv
+    import glob
+    la_lb = {"ss": "0, 0", "ps": "1, 0", "pp": "1, 1", "ds": "2, 0", "dp": "2, 1", "dd": "2, 2", "fs": "3, 0", "fp": "3, 1",
+             "fd": "3, 2", "ff": "3, 3"}[cls_name]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_full_cfg%d.csv" % cfg)), reverse=True):
+        try:
+            with open(path, newline="") as f:
+                rows = list(csv.reader(f))
+            hdr = rows[0]
+            col = {h.split("[")[0]: (i, (h.split("[")[1][:-1] if "[" in h else "")) for i, h in enumerate(hdr)}
+            for r in rows[1:]:
+                if "k_integrals<%s>" % la_lb in r[col["kernel"][0]]:
+                    return sum(float(r[col[k][0]]) * scale.get(col[k][1], 1.0) for k in ("dram_read", "dram_write"))
+        except Exception:
+            continue
     return None
 
 

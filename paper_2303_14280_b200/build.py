@@ -11,6 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "csrc", "build")
 LIB = os.path.join(HERE, "libsnk.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+NVCC_FLAGS += os.environ.get("SNK_NVCC_FLAGS", "").split()     # e.g. -DSNK_NP2_MAXL=1 -Xptxas -v (kernel tuning)
 
 
 def sources():

@@ -552,7 +552,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   CK(ctx->d_units.reserve((size_t)std::max(nunit, 1) * kUnitBytes)); CK(ctx->d_meta.reserve(std::max(nunit, 1)));
   CK(ctx->d_vmask.reserve((size_t)nb * ctx->vstride));
   CK(run_unit_fill(ctx->cand, tab, ctx->d_flag.p, ctx->d_pos.p, ctx->d_Atil.p, 1e-4 * ctx->eps, (const double*)ctx->d_Fmax.p,
-                   (const double*)ctx->d_phimax.p, ctx->d_units.p, ctx->d_meta.p, s));
+                   (const double*)ctx->d_phimax.p, ctx->ld, ctx->d_units.p, ctx->d_meta.p, s));
   CK(cudaMemsetAsync(ctx->d_vmask.p, 0, (size_t)nb * ctx->vstride * sizeof(uint32_t), s));
   CK(run_vmask(nb, nunit, ctx->d_meta.p, ctx->d_FtsT.p, nsh, ctx->d_phit.p, ctx->eps, ctx->d_vmask.p, ctx->vstride, s));
   ctx->n_launches += 6;

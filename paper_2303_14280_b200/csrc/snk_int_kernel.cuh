@@ -18,11 +18,16 @@
 
 namespace snk {
 
-// points per consumer thread: two for the low-L classes (their registers allow it), one otherwise
-__host__ __device__ constexpr int int_npmax(int LA, int LB) { return 1; }
-// resident CTAs per SM the register allocation is held to (the kernel is latency bound: warps in flight matter most)
+// points per consumer thread: two for the low-L classes (two independent recurrence streams per thread cover the 8-cycle
+// FP64 latency and halve the per-unit bookkeeping per point), one where the registers do not allow it
+#ifndef SNK_NP2_MAXL
+#define SNK_NP2_MAXL -1
+#endif
+__host__ __device__ constexpr int int_npmax(int LA, int LB) { return LA + LB <= SNK_NP2_MAXL ? 2 : 1; }
+// resident CTAs per SM the register allocation is held to
 __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
   const int L = LA + LB;
+  if (int_npmax(LA, LB) == 2) return L == 0 ? 8 : L == 1 ? 5 : L == 2 ? 4 : 3;
   return L == 0 ? 7 : L == 1 ? 4 : L == 2 ? 4 : L == 3 ? 3 : L == 4 ? 2 : 1;
 }
 __host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile / int_npmax(LA, LB) + 32; }
@@ -54,22 +59,35 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-// producer-side wait: poll with back-off so that the waiting lane does not steal issue slots from the consumer warps
-__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+// producer-side wait: try_wait suspends the lane in hardware until the phase completes or the time hint (ns) expires, so the
+// waiting producer takes (almost) no issue slots from the consumer warps
+__device__ __forceinline__ void mbar_wait_suspend(uint32_t bar, uint32_t parity) {
   uint32_t done;
-  for (;;) {
+  do {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
         "selp.u32 %0, 1, 0, p;\n"
         "}\n"
         : "=r"(done)
-        : "r"(bar), "r"(parity)
+        : "r"(bar), "r"(parity), "r"(1000000u)
         : "memory");
-    if (done) break;
-    __nanosleep(200);
-  }
+  } while (!done);
+}
+// non-blocking probe (the consumer issues it one unit ahead, so the barrier round trip overlaps the recurrences)
+__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(done)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return done;
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
@@ -101,35 +119,44 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
   const int64_t ld = p.ld;
 
   int cur_fa = -1;
+  int64_t cur_offa = 0;
   double Fa[NP][NA], Ga[NP][NA];
 #pragma unroll
   for (int s = 0; s < NP; ++s)
 #pragma unroll
     for (int i = 0; i < NA; ++i) { Fa[s][i] = 0.0; Ga[s][i] = 0.0; }
 
+  auto flush_a = [&]() {
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+      if (act[s]) {
+#pragma unroll
+        for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + cur_offa + (int64_t)i * ld, Ga[s][i]);
+      }
+  };
+
   uint32_t sl = 0, phase = 0;
+  uint32_t ready = mbar_test(s_full, 0);
   for (;;) {
-    mbar_wait(s_full + 8 * sl, phase);
+    if (!ready) mbar_wait(s_full + 8 * sl, phase);
     const unsigned char* rec = smem_int + sl * SLOT;
     const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
     const int fa = h0.x, fb = h0.y;
     if (fa < 0) break;
+    // probe the next slot's barrier now: its round trip overlaps this unit's recurrences
+    uint32_t nsl = sl + 1, nphase = phase;
+    if (nsl == NS) { nsl = 0; nphase ^= 1; }
+    ready = mbar_test(s_full + 8 * nsl, nphase);
     const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
     const double ABz = *reinterpret_cast<const double*>(rec + 32);
+    const longlong2 off = *reinterpret_cast<const longlong2*>(rec + 48);   // fa * ld, fb * ld
     if (fa != cur_fa) {
-      if (cur_fa >= 0) {
-#pragma unroll
-        for (int s = 0; s < NP; ++s)
-          if (act[s]) {
-#pragma unroll
-            for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + (int64_t)(cur_fa + i) * ld, Ga[s][i]);
-          }
-      }
-      cur_fa = fa;
+      if (cur_fa >= 0) flush_a();
+      cur_fa = fa; cur_offa = off.x;
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[s][(int64_t)(fa + i) * ld]; Ga[s][i] = 0.0; }
+        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[s][off.x + (int64_t)i * ld]; Ga[s][i] = 0.0; }
     }
     double Fb[NP][NB], Gb[NP][NB];
     const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
@@ -148,24 +175,17 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
-    if (++sl == NS) { sl = 0; phase ^= 1; }
+    sl = nsl; phase = nphase;
     if (fa != fb) {                                                // a == b (same shell): one direction only
 #pragma unroll
       for (int s = 0; s < NP; ++s)
         if (act[s]) {
 #pragma unroll
-          for (int k = 0; k < NB; ++k) atomicAdd(Gc[s] + (int64_t)(fb + k) * ld, Gb[s][k]);
+          for (int k = 0; k < NB; ++k) atomicAdd(Gc[s] + off.y + (int64_t)k * ld, Gb[s][k]);
         }
     }
   }
-  if (cur_fa >= 0) {
-#pragma unroll
-    for (int s = 0; s < NP; ++s)
-      if (act[s]) {
-#pragma unroll
-        for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + (int64_t)(cur_fa + i) * ld, Ga[s][i]);
-      }
-  }
+  if (cur_fa >= 0) flush_a();
 }
 
 template <int LA, int LB>
@@ -215,7 +235,7 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
           // slots are released in unit order, so the step's last slot being free implies the others are: one lane polls
           if (lane == 0) {
             const uint32_t last = u + (uint32_t)cnt - 1u;
-            if (last >= NS) mbar_wait_backoff(s_empty + 8 * (last % NS), (last / NS - 1) & 1);
+            if (last >= NS) mbar_wait_suspend(s_empty + 8 * (last % NS), (last / NS - 1) & 1);
           }
           __syncwarp();
           if (mine) {
@@ -235,7 +255,7 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
     }
     if (lane == 0) {                                       // end-of-list sentinel: a header with fa = -1
       const uint32_t slot = u % NS, round = u / NS;
-      if (round > 0) mbar_wait_backoff(s_empty + 8 * slot, (round - 1) & 1);
+      if (round > 0) mbar_wait_suspend(s_empty + 8 * slot, (round - 1) & 1);
       reinterpret_cast<volatile int32_t*>(smem_int + slot * SLOT)[0] = -1;
       mbar_arrive(s_full + 8 * slot);
     }

@@ -31,8 +31,7 @@ struct __align__(16) UnitHdr {
   int32_t first;          // 1 for the first unit of its pair
   double ABx, ABy, ABz;   // A - B
   int32_t sa, sb;         // shell ids
-  double At;              // R11 bound of the pair
-  int32_t pad[2];
+  int64_t offa, offb;     // fa * ld, fb * ld: element offsets of the shells' first rows in the F / G slabs
 };
 static_assert(sizeof(UnitHdr) == 64, "UnitHdr layout");
 constexpr int kPrimBytes = 80;                                   // sizeof(PrimPair), snk_os.cuh

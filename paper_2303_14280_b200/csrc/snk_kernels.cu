@@ -323,7 +323,8 @@ __global__ void k_pair_flags(PairCand pc, ShellTab sh, const double* __restrict_
 // pair's units in order; trailing units may stay empty (nprim = 0) and are then never part of V_j.
 __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict__ nunit, const int32_t* __restrict__ pos,
                             const double* __restrict__ Atil, double prim_thresh, const double* __restrict__ Fmax,
-                            const double* __restrict__ phimax, unsigned char* __restrict__ units, UnitMeta* __restrict__ meta) {
+                            const double* __restrict__ phimax, int64_t ld, unsigned char* __restrict__ units,
+                            UnitMeta* __restrict__ meta) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= pc.off[kNumClasses] || nunit[i] == 0) return;
   int a, b;
@@ -362,7 +363,7 @@ __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict_
     const int np = max(0, min(kUnitPrims, n - u * kUnitPrims));
     UnitHdr h;
     h.fa = sh.foff[a]; h.fb = sh.foff[b]; h.nprim = np; h.first = u == 0;
-    h.ABx = ABx; h.ABy = ABy; h.ABz = ABz; h.sa = a; h.sb = b; h.At = At; h.pad[0] = h.pad[1] = 0;
+    h.ABx = ABx; h.ABy = ABy; h.ABz = ABz; h.sa = a; h.sb = b; h.offa = (int64_t)h.fa * ld; h.offb = (int64_t)h.fb * ld;
     *reinterpret_cast<UnitHdr*>(units + (size_t)(u0 + u) * kUnitBytes) = h;
     UnitMeta m;
     m.sa = a; m.sb = b; m.fb = h.fb; m.nprim_first = np | ((u == 0) << 8); m.At = At;
@@ -560,10 +561,10 @@ cudaError_t run_pair_flags(const PairCand& pc, const ShellTab& sh, const double*
 }
 
 cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t* nunit, const int32_t* pos, const double* Atil,
-                          double prim_thresh, const double* Fmax, const double* phimax, unsigned char* units, UnitMeta* meta,
-                          cudaStream_t s) {
+                          double prim_thresh, const double* Fmax, const double* phimax, int64_t ld, unsigned char* units,
+                          UnitMeta* meta, cudaStream_t s) {
   const int64_t n = pc.off[kNumClasses];
-  if (n > 0) k_unit_fill<<<nblk(n, 128), 128, 0, s>>>(pc, sh, nunit, pos, Atil, prim_thresh, Fmax, phimax, units, meta);
+  if (n > 0) k_unit_fill<<<nblk(n, 128), 128, 0, s>>>(pc, sh, nunit, pos, Atil, prim_thresh, Fmax, phimax, ld, units, meta);
   return cudaGetLastError();
 }
 

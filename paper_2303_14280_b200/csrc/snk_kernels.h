@@ -38,8 +38,8 @@ cudaError_t run_shell_max(const ShellTab& sh, int nbatch, const double* Ftf, int
 cudaError_t run_pair_flags(const PairCand& pc, const ShellTab& sh, const double* Atil, const double* Fmax, const double* phimax, double eps,
                            int32_t* nunit, int32_t* ispair, cudaStream_t s);
 cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t* nunit, const int32_t* pos, const double* Atil,
-                          double prim_thresh, const double* Fmax, const double* phimax, unsigned char* units, UnitMeta* meta,
-                          cudaStream_t s);
+                          double prim_thresh, const double* Fmax, const double* phimax, int64_t ld, unsigned char* units,
+                          UnitMeta* meta, cudaStream_t s);
 cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
                       uint32_t* vmask, int64_t vstride, cudaStream_t s);
 cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
