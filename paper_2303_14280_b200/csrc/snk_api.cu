@@ -748,7 +748,7 @@ int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double
       q.Px = (za * A[0] + zb * B[0]) / q.p; q.Py = (za * A[1] + zb * B[1]) / q.p; q.Pz = (za * A[2] + zb * B[2]) / q.p;
       q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
       q.pref = ctx->h_pcoef[ctx->h_poff[sa] + k] * ctx->h_pcoef[ctx->h_poff[sb] + l] * (2.0 * M_PI / q.p) * std::exp(-(za * zb / q.p) * AB2);
-      q.pad = 0.0;
+      q.cfar = 0.88622692545275801365 * q.pref;
       pp.push_back(q);
     }
   DevBuf<PrimPair> d;

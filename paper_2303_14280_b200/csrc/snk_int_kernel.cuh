@@ -32,7 +32,13 @@ __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
 }
 __host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile / int_npmax(LA, LB) + 32; }
 
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : 8; }
+#ifndef SNK_NS_LB0
+#define SNK_NS_LB0 8
+#endif
+#ifndef SNK_NS_LB1
+#define SNK_NS_LB1 8
+#endif
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8; }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
 __host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB); }
 

@@ -355,7 +355,7 @@ __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict_
       q.Px = (za * A[0] + zb * B[0]) / q.p; q.Py = (za * A[1] + zb * B[1]) / q.p; q.Pz = (za * A[2] + zb * B[2]) / q.p;
       q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
       q.pref = ca * cb * (6.283185307179586 / q.p) * exp(-(za * zb / q.p) * AB2);
-      q.pad = 0.0;
+      q.cfar = 0.88622692545275801365 * q.pref;   // pref sqrt(pi)/2: far-field seed constant
       *reinterpret_cast<PrimPair*>(units + (size_t)(u0 + n / kUnitPrims) * kUnitBytes + 64 + (n % kUnitPrims) * kPrimBytes) = q;
       ++n;
     }

@@ -114,6 +114,61 @@ __device__ __forceinline__ void boys_near(double x, const double* __restrict__ t
   }
 }
 
+// Seeds (A3, R1) Theta^n_0 = pref F_n(x), n = 0..L, with the prefactor folded into the Boys evaluation:
+// far field: Theta^0_0 = cfar / sqrt(x), cfar = pref sqrt(pi)/2, and Theta^{m+1}_0 = Theta^m_0 (2m+1)/(2x): the factors
+// (2m+1) h are formed off the critical path; near field: pref scales F_L and e^{-x} once, the downward recursion is linear.
+template <int L>
+__device__ __forceinline__ void seeds_far(double x, double cfar, double (&T)[L + 1]) {
+  double y0;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+  const double e = fma(-x, y0 * y0, 1.0);
+  const double r = fma(fma(e, 0.375, 0.5), y0 * e, y0);
+  T[0] = cfar * r;
+  if constexpr (L > 0) {
+    const double h = (0.5 * r) * r;                // 1/(2x)
+    T[1] = T[0] * h;
+#pragma unroll
+    for (int m = 1; m < L; ++m) T[m + 1] = T[m] * ((2 * m + 1) * h);
+  }
+}
+template <int L>
+__device__ __forceinline__ void seeds_near(double x, double pref, const double* __restrict__ tab, double (&T)[L + 1]) {
+  const double tm = fma(x, 16.0, 6755399441055744.0);
+  const int i = __double2loint(tm);
+  const double d = fma(tm - 6755399441055744.0, kBoysDelta, -x);
+  const double2* __restrict__ row = reinterpret_cast<const double2*>(tab + ((size_t)L * kBoysRows + i) * kBoysStride);
+  const double2 t01 = __ldg(row), t23 = __ldg(row + 1), t45 = __ldg(row + 2), t67 = __ldg(row + 3);
+  double s = fma(t67.y, d, t67.x);
+  s = fma(s, d, t45.y);
+  s = fma(s, d, t45.x);
+  s = fma(s, d, t23.y);
+  s = fma(s, d, t23.x);
+  s = fma(s, d, t01.y);
+  s = fma(s, d, t01.x);
+  T[L] = s * pref;
+  if constexpr (L > 0) {
+    const double2 e = __ldg(row + 4);
+    const double ep = e.x * pref;
+    double q = 1.0 / 5040.0;
+    q = fma(q, d, 1.0 / 720.0);
+    q = fma(q, d, 1.0 / 120.0);
+    q = fma(q, d, 1.0 / 24.0);
+    q = fma(q, d, 1.0 / 6.0);
+    q = fma(q, d, 0.5);
+    q = fma(q, d, 1.0);
+    q = fma(q, d, 1.0);
+    const double ex = ep * q;
+    const double x2 = x + x;
+#pragma unroll
+    for (int m = L; m >= 1; --m) T[m - 1] = fma(x2, T[m], ex) * (1.0 / (2 * m - 1));
+  }
+}
+template <int L>
+__device__ __forceinline__ void seeds(double x, double pref, double cfar, const double* __restrict__ tab, double (&T)[L + 1]) {
+  if (x < boys_xmax(L)) seeds_near<L>(x, pref, tab, T);
+  else seeds_far<L>(x, cfar, T);
+}
+
 // per-lane dispatch (test hooks, divergent warps)
 template <int L>
 __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, double (&F)[L + 1]) {
@@ -130,7 +185,7 @@ struct __align__(16) PrimPair {
   double Px, Py, Pz;
   double PAx, PAy, PAz;   // P - A, A = centre of the shell that carries the VRR (first of the pair, l_a >= l_b)
   double pref;     // c_a c_b (2 pi / p) exp(-zeta_a zeta_b / p |A-B|^2)
-  double pad;
+  double cfar;     // pref * sqrt(pi)/2: Theta^0_0 = cfar / sqrt(x) in the far field
 };
 static_assert(sizeof(PrimPair) == 80, "PrimPair layout");
 
@@ -166,13 +221,24 @@ __device__ __forceinline__ void vrr_accumulate(const double (&th0)[L + 1], doubl
         constexpr int aq = q == 0 ? li : (q == 1 ? lj : lk);     // a_q: quantum before raising
         const double PAq = q == 0 ? PAx : (q == 1 ? PAy : PAz);
         const double PCq = q == 0 ? PCx : (q == 1 ? PCy : PCz);
-        double t = fma(PAq, v[o0 + n * nc0 + cl], -PCq * v[o0 + (n + 1) * nc0 + cl]);
-        if constexpr (aq > 0) {
-          constexpr int cll = cidx(li - (q == 0), lj - (q == 1), lk - (q == 2));
-          t = fma((double)aq * inv2p, v[om + n * ncm + cll] - v[om + (n + 1) * ncm + cll], t);
+        if constexpr (l + 1 == L) {
+          // top level: the value feeds nothing but the contraction sum (R4), so its terms go straight into acc
+          double a = fma(PAq, v[o0 + n * nc0 + cl], acc[nlev(LA, l) + c]);
+          a = fma(-PCq, v[o0 + (n + 1) * nc0 + cl], a);
+          if constexpr (aq > 0) {
+            constexpr int cll = cidx(li - (q == 0), lj - (q == 1), lk - (q == 2));
+            a = fma((double)aq * inv2p, v[om + n * ncm + cll] - v[om + (n + 1) * ncm + cll], a);
+          }
+          acc[nlev(LA, l) + c] = a;
+        } else {
+          double t = fma(PAq, v[o0 + n * nc0 + cl], -PCq * v[o0 + (n + 1) * nc0 + cl]);
+          if constexpr (aq > 0) {
+            constexpr int cll = cidx(li - (q == 0), lj - (q == 1), lk - (q == 2));
+            t = fma((double)aq * inv2p, v[om + n * ncm + cll] - v[om + (n + 1) * ncm + cll], t);
+          }
+          v[o1 + n * nc1 + c] = t;
+          if constexpr (n == 0 && l + 1 >= LA) acc[nlev(LA, l) + c] += t;
         }
-        v[o1 + n * nc1 + c] = t;
-        if constexpr (n == 0 && l + 1 >= LA) acc[nlev(LA, l) + c] += t;
       });
     });
   });
@@ -281,32 +347,30 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
     }
     bool allfar = false;
     if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
+    double2 q4[K];                                    // (pref, cfar)
+#pragma unroll
+    for (int j = 0; j < K; ++j) q4[j] = reinterpret_cast<const double2*>(pp + k + j)[4];
     if (allfar) {
 #pragma unroll
       for (int j = 0; j < K; ++j)
 #pragma unroll
-        for (int s = 0; s < NP; ++s) boys_far<L>(x[j][s], th0[j][s]);
+        for (int s = 0; s < NP; ++s) seeds_far<L>(x[j][s], q4[j].y, th0[j][s]);
     } else {
 #pragma unroll
       for (int j = 0; j < K; ++j)
 #pragma unroll
-        for (int s = 0; s < NP; ++s) boys<L>(x[j][s], boys_tab, th0[j][s]);
+        for (int s = 0; s < NP; ++s) seeds<L>(x[j][s], q4[j].x, q4[j].y, boys_tab, th0[j][s]);
     }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
-      const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k + j);
-      const double2 q4 = q[4];                        // (pref, pad)
       if constexpr (L == 0) {
 #pragma unroll
-        for (int s = 0; s < NP; ++s) acc[s][0] = fma(th0[j][s][0], q4.x, acc[s][0]);
+        for (int s = 0; s < NP; ++s) acc[s][0] += th0[j][s][0];
       } else {
-        const double2 q3 = q[3];                      // (PAy, PAz)
+        const double2 q3 = reinterpret_cast<const double2*>(pp + k + j)[3];   // (PAy, PAz)
 #pragma unroll
-        for (int s = 0; s < NP; ++s) {
-#pragma unroll
-          for (int n = 0; n <= L; ++n) th0[j][s][n] *= q4.x;
+        for (int s = 0; s < NP; ++s)
           vrr_accumulate<LA, L>(th0[j][s], q2[j].y, q3.x, q3.y, PCx[j][s], PCy[j][s], PCz[j][s], q0[j].y, acc[s]);
-        }
       }
     }
   };
@@ -330,25 +394,21 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
       }
       bool allfar = false;
       if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
+      const double2 q4 = q[4];                          // (pref, cfar)
       if (allfar) {
 #pragma unroll
-        for (int s = 0; s < NP; ++s) boys_far<L>(x[s], th0[s]);
+        for (int s = 0; s < NP; ++s) seeds_far<L>(x[s], q4.y, th0[s]);
       } else {
 #pragma unroll
-        for (int s = 0; s < NP; ++s) boys<L>(x[s], boys_tab, th0[s]);
+        for (int s = 0; s < NP; ++s) seeds<L>(x[s], q4.x, q4.y, boys_tab, th0[s]);
       }
-      const double2 q4 = q[4];                          // (pref, pad)
       if constexpr (L == 0) {
 #pragma unroll
-        for (int s = 0; s < NP; ++s) acc[s][0] = fma(th0[s][0], q4.x, acc[s][0]);
+        for (int s = 0; s < NP; ++s) acc[s][0] += th0[s][0];
       } else {
         const double2 q3 = q[3];                        // (PAy, PAz)
 #pragma unroll
-        for (int s = 0; s < NP; ++s) {
-#pragma unroll
-          for (int n = 0; n <= L; ++n) th0[s][n] *= q4.x;
-          vrr_accumulate<LA, L>(th0[s], q2.y, q3.x, q3.y, PCx[s], PCy[s], PCz[s], q0.y, acc[s]);
-        }
+        for (int s = 0; s < NP; ++s) vrr_accumulate<LA, L>(th0[s], q2.y, q3.x, q3.y, PCx[s], PCy[s], PCz[s], q0.y, acc[s]);
       }
     }
   }
