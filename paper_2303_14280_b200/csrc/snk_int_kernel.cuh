@@ -7,10 +7,12 @@
 //     every kept pair unit -- header + primitive pairs (<= 704 B) and the F_b rows of this tile -- into a ring of
 //     shared-memory slots with cp.async.bulk (TMA bulk copy) completing on an mbarrier; consumers never touch pair
 //     data in global memory, so the recurrences run against broadcast LDS only;
+//   * a consumer thread owns NP points of the tile (4 for L <= 1, 2 for L = 2, else 1) and the NP warps that cover the
+//     same points split the unit stream dynamically (shared-memory ticket): the point-independent work of a unit is
+//     paid once per 32 NP points;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
 //     fire-and-forget RED.F64 (coalesced along the slot index);
-//   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh);
-//   * consumer warps with no point of the tile retire immediately.
+//   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh).
 // Included once per (LA,LB) translation unit.
 #pragma once
 #include "snk_internal.h"
@@ -18,19 +20,45 @@
 
 namespace snk {
 
-// points per consumer thread: two for the low-L classes (two independent recurrence streams per thread cover the 8-cycle
-// FP64 latency and halve the per-unit bookkeeping per point), one where the registers do not allow it
-#ifndef SNK_NP2_MAXL
-#define SNK_NP2_MAXL -1
+// Work split inside a CTA (one tile of up to kTile points, four consumer warps + one producer warp).
+// A consumer thread holds NP = int_npmax points of the tile (lane, lane + 32, ...): everything that does not depend on the grid
+// point -- the broadcast LDS of the primitive pairs, the loop and barrier bookkeeping -- is paid once per NP points, and the
+// NP recurrences are independent instruction streams.  The tile is therefore covered by G = 4 / NP point groups of NP warps
+// each, and the warps of one group share the unit stream: each takes the next unit nobody of its group has taken yet.
+#ifndef SNK_NP_L0
+#define SNK_NP_L0 4
 #endif
-__host__ __device__ constexpr int int_npmax(int LA, int LB) { return LA + LB <= SNK_NP2_MAXL ? 2 : 1; }
+#ifndef SNK_NP_L1
+#define SNK_NP_L1 4
+#endif
+#ifndef SNK_NP_L2
+#define SNK_NP_L2 2
+#endif
+#ifndef SNK_NP_L3
+#define SNK_NP_L3 1
+#endif
+__host__ __device__ constexpr int int_npmax(int LA, int LB) {
+  const int L = LA + LB;
+  return L == 0 ? SNK_NP_L0 : L == 1 ? SNK_NP_L1 : L == 2 ? SNK_NP_L2 : L == 3 ? SNK_NP_L3 : 1;
+}
 // resident CTAs per SM the register allocation is held to
+#ifndef SNK_MB_L0
+#define SNK_MB_L0 4
+#endif
+#ifndef SNK_MB_L1
+#define SNK_MB_L1 3
+#endif
+#ifndef SNK_MB_L2
+#define SNK_MB_L2 3
+#endif
+#ifndef SNK_MB_L3
+#define SNK_MB_L3 3
+#endif
 __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
   const int L = LA + LB;
-  if (int_npmax(LA, LB) == 2) return L == 0 ? 8 : L == 1 ? 5 : L == 2 ? 4 : 3;
-  return L == 0 ? 7 : L == 1 ? 4 : L == 2 ? 4 : L == 3 ? 3 : L == 4 ? 2 : 1;
+  return L == 0 ? SNK_MB_L0 : L == 1 ? SNK_MB_L1 : L == 2 ? SNK_MB_L2 : L == 3 ? SNK_MB_L3 : L == 4 ? 2 : 1;
 }
-__host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile / int_npmax(LA, LB) + 32; }
+__host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile + 32; }
 
 #ifndef SNK_NS_LB0
 #define SNK_NS_LB0 8
@@ -40,7 +68,8 @@ __host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile / i
 #endif
 __host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8; }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
-__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB); }
+// ring slots, then full[NS] and empty[NS] mbarriers, then the per-group unit counters and the unit count
+__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB) + 32; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -101,10 +130,11 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                : "memory");
 }
 
-// ---- consumer side: the whole unit stream for the 32*NP points [pbase, pbase + 32 NP) of the tile, NP points per thread ----
+// ---- consumer side: this warp's share of the unit stream for the points [pbase, pbase + 32 NP) of the tile, NP per thread ----
+// s_next: shared counter of the warp's point group (next unit nobody of the group has taken); nunit: units of the tile's stream.
 template <int LA, int LB, int NP>
 __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned char* smem_int, uint32_t s_full, uint32_t s_empty,
-                                              const TileRec& tile, int64_t col0, int pbase, int lane) {
+                                              int* s_next, int nunit, const TileRec& tile, int64_t col0, int pbase, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
   constexpr int NS = int_nslots(LA, LB), SLOT = int_slot_bytes(LB);
   int pt[NP], ptc[NP];
@@ -118,10 +148,8 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
     const int64_t slot = tile.slot + ptc[s];
     gx[s] = p.gx[slot]; gy[s] = p.gy[slot]; gz[s] = p.gz[slot];
   }
-  const double* __restrict__ Fc[NP];
-  double* __restrict__ Gc[NP];
-#pragma unroll
-  for (int s = 0; s < NP; ++s) { Fc[s] = p.F + col0 + ptc[s]; Gc[s] = p.G + col0 + pt[s]; }
+  const double* __restrict__ Fc = p.F + col0;
+  double* __restrict__ Gc = p.G + col0;
   const int64_t ld = p.ld;
 
   int cur_fa = -1;
@@ -137,22 +165,23 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
     for (int s = 0; s < NP; ++s)
       if (act[s]) {
 #pragma unroll
-        for (int i = 0; i < NA; ++i) atomicAdd(Gc[s] + cur_offa + (int64_t)i * ld, Ga[s][i]);
+        for (int i = 0; i < NA; ++i) atomicAdd(Gc + cur_offa + (int64_t)i * ld + pt[s], Ga[s][i]);
       }
   };
 
-  uint32_t sl = 0, phase = 0;
-  uint32_t ready = mbar_test(s_full, 0);
-  for (;;) {
-    if (!ready) mbar_wait(s_full + 8 * sl, phase);
+  auto take = [&]() {                                  // next unit of the group's stream
+    int u = 0;
+    if (lane == 0) u = atomicAdd(s_next, 1);
+    return __shfl_sync(0xffffffffu, u, 0);
+  };
+  int u = take();
+  while (u < nunit) {
+    const uint32_t sl = (uint32_t)u % NS, phase = ((uint32_t)u / NS) & 1u;
+    if (!mbar_test(s_full + 8 * sl, phase)) mbar_wait(s_full + 8 * sl, phase);
+    const int unext = take();                          // the shared-memory round trip overlaps this unit's recurrences
     const unsigned char* rec = smem_int + sl * SLOT;
     const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
     const int fa = h0.x, fb = h0.y;
-    if (fa < 0) break;
-    // probe the next slot's barrier now: its round trip overlaps this unit's recurrences
-    uint32_t nsl = sl + 1, nphase = phase;
-    if (nsl == NS) { nsl = 0; nphase ^= 1; }
-    ready = mbar_test(s_full + 8 * nsl, nphase);
     const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
     const double ABz = *reinterpret_cast<const double*>(rec + 32);
     const longlong2 off = *reinterpret_cast<const longlong2*>(rec + 48);   // fa * ld, fb * ld
@@ -162,7 +191,7 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[s][off.x + (int64_t)i * ld]; Ga[s][i] = 0.0; }
+        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[off.x + (int64_t)i * ld + ptc[s]]; Ga[s][i] = 0.0; }
     }
     double Fb[NP][NB], Gb[NP][NB];
     const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
@@ -181,15 +210,15 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
-    sl = nsl; phase = nphase;
     if (fa != fb) {                                                // a == b (same shell): one direction only
 #pragma unroll
       for (int s = 0; s < NP; ++s)
         if (act[s]) {
 #pragma unroll
-          for (int k = 0; k < NB; ++k) atomicAdd(Gc[s] + off.y + (int64_t)k * ld, Gb[s][k]);
+          for (int k = 0; k < NB; ++k) atomicAdd(Gc + off.y + (int64_t)k * ld + pt[s], Gb[s][k]);
         }
     }
+    u = unext;
   }
   if (cur_fa >= 0) flush_a();
 }
@@ -197,34 +226,49 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 template <int LA, int LB>
 __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_integrals(IntParams p) {
   constexpr int NB = ncart(LB);
-  constexpr int NPM = int_npmax(LA, LB), CW = kTile / (32 * NPM);   // points per thread, consumer warps per CTA
+  constexpr int NPM = int_npmax(LA, LB), CW = kTile / 32;           // points per thread, consumer warps per CTA
   constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
+  static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
   const uint32_t s_base = smem_u32(smem_int);
   const uint32_t s_full = s_base + NS * SLOT, s_empty = s_full + NS * 8;
+  int* s_ctr = reinterpret_cast<int*>(smem_int + NS * SLOT + 16 * NS);   // [0..3] next unit of point group g, [4] units of the tile
 
   const TileRec tile = p.tiles[blockIdx.x];
   const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-  const int nw = (tile.n + 32 * NPM - 1) / (32 * NPM);     // consumer warps that own at least one point
-  const int npad = ((tile.n + 31) >> 5) << 5;
+  const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
+  const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
+  auto class_bits = [&](int w) {                           // V_j bits of word w that belong to this class
+    uint32_t word = __ldg(mask + w);
+    if (w == w0) word &= 0xffffffffu << (p.pbeg & 31);
+    if (w == w1 - 1 && (p.pend & 31)) word &= 0xffffffffu >> (32 - (p.pend & 31));
+    return word;
+  };
+  // length of the tile's unit stream
+  int cnt = 0;
+  for (int w = w0 + t; w < w1; w += int_threads(LA, LB)) cnt += __popc(class_bits(w));
+  cnt = __reduce_add_sync(0xffffffffu, cnt);
+  if (t < 8) s_ctr[t] = 0;
+  __syncthreads();
+  if (lane == 0 && cnt) atomicAdd(s_ctr + 4, cnt);
+  const int nag = (tile.n + 32 * NPM - 1) / (32 * NPM);    // point groups that own at least one point
   if (t == 0) {
-    for (int i = 0; i < NS; ++i) { mbar_init(s_full + 8 * i, 1); mbar_init(s_empty + 8 * i, nw); }
+    for (int i = 0; i < NS; ++i) { mbar_init(s_full + 8 * i, 1); mbar_init(s_empty + 8 * i, nag); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  const int nunit = s_ctr[4];
+  if (nunit == 0) return;
   const int64_t col0 = tile.slot - p.slot0;
 
   if (warp == CW) {
     // ------------------------------------------------ producer warp ------------------------------------------------
-    const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
-    const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
+    const int npad = ((tile.n + 31) >> 5) << 5;
     const uint32_t frow = (uint32_t)npad * 8u;             // bytes of one staged F row
     uint32_t u = 0;                                        // units issued so far
     for (int wb = w0; wb < w1; wb += 32) {
       const int w = wb + lane;
-      uint32_t word = w < w1 ? __ldg(mask + w) : 0u;
-      if (w == w0) word &= 0xffffffffu << (p.pbeg & 31);
-      if (w == w1 - 1 && (p.pend & 31)) word &= 0xffffffffu >> (32 - (p.pend & 31));
+      const uint32_t word = w < w1 ? class_bits(w) : 0u;
       uint32_t any = __ballot_sync(~0u, word != 0u);
       while (any) {
         const int src = __ffs(any) - 1;
@@ -233,19 +277,13 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
         const int n = __popc(bits);
         const int base_pid = (wb + src) << 5;
         for (int b0 = 0; b0 < n; b0 += NG) {               // NG units per step (half the ring): one lane per unit
-          const int cnt = min(n, b0 + NG) - b0;
-          const bool mine = lane >= b0 && lane < b0 + cnt;
-          int pid = 0;
-          UnitMeta m{};
-          if (mine) { pid = base_pid + (int)__fns(bits, 0, lane + 1); m = p.meta[pid]; }   // in flight while we wait for slots
-          // slots are released in unit order, so the step's last slot being free implies the others are: one lane polls
-          if (lane == 0) {
-            const uint32_t last = u + (uint32_t)cnt - 1u;
-            if (last >= NS) mbar_wait_suspend(s_empty + 8 * (last % NS), (last / NS - 1) & 1);
-          }
-          __syncwarp();
-          if (mine) {
-            const uint32_t slot = (u + (uint32_t)(lane - b0)) % NS;
+          const int cnt_step = min(n, b0 + NG) - b0;
+          if (lane >= b0 && lane < b0 + cnt_step) {
+            const int pid = base_pid + (int)__fns(bits, 0, lane + 1);
+            const UnitMeta m = p.meta[pid];                // in flight while we wait for the slot
+            const uint32_t uu = u + (uint32_t)(lane - b0), slot = uu % NS;
+            // the slot's previous unit is released by the one warp of every point group that processed it
+            if (uu >= NS) mbar_wait_suspend(s_empty + 8 * slot, (uu / NS - 1) & 1);
             const uint32_t nb = 64u + (uint32_t)(m.nprim_first & 0xff) * (uint32_t)kPrimBytes;
             const uint32_t bar = s_full + 8 * slot, dst = s_base + slot * SLOT;
             mbar_arrive_expect_tx(bar, nb + NB * frow);
@@ -254,26 +292,27 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
 #pragma unroll
             for (int k = 0; k < NB; ++k) bulk_g2s(dst + kUnitBytes + k * (kTile * 8), Fsrc + (int64_t)k * p.ld, frow, bar);
           }
-          u += (uint32_t)cnt;
+          u += (uint32_t)cnt_step;
           __syncwarp();
         }
       }
     }
-    if (lane == 0) {                                       // end-of-list sentinel: a header with fa = -1
-      const uint32_t slot = u % NS, round = u / NS;
-      if (round > 0) mbar_wait_suspend(s_empty + 8 * slot, (round - 1) & 1);
-      reinterpret_cast<volatile int32_t*>(smem_int + slot * SLOT)[0] = -1;
-      mbar_arrive(s_full + 8 * slot);
-    }
     return;
   }
-  if (warp >= nw) return;
-  const int pbase = warp * 32 * NPM;
-  if constexpr (NPM == 2) {
-    if (tile.n - pbase <= 32) consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);   // ragged tail: one point per thread
-    else consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);
+  const int grp = warp / NPM, pbase = grp * 32 * NPM;
+  if (pbase >= tile.n) return;
+  const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
+  int* s_next = s_ctr + grp;
+  if constexpr (NPM == 4) {
+    if (need == 4) consume_units<LA, LB, 4>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    else if (need == 3) consume_units<LA, LB, 3>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    else if (need == 2) consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    else consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+  } else if constexpr (NPM == 2) {
+    if (need == 2) consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    else consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
   } else {
-    consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, tile, col0, pbase, lane);
+    consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
   }
 }
 

@@ -131,6 +131,41 @@ __device__ __forceinline__ void seeds_far(double x, double cfar, double (&T)[L +
     for (int m = 1; m < L; ++m) T[m + 1] = T[m] * ((2 * m + 1) * h);
   }
 }
+// The same for N independent (primitive pair, point) arguments, written statement by statement across the N streams: the
+// warp issues in order, so consecutive instructions must belong to different dependency chains to cover the 8-cycle FP64
+// latency (a Newton step per point in sequence would stall on every instruction).
+template <int L, int N>
+__device__ __forceinline__ void seeds_far_v(const double (&x)[N], const double (&cfar)[N], double (&T)[N][L + 1]) {
+  double y0[N], e[N], u[N], r[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0[i]) : "d"(x[i]));
+#pragma unroll
+  for (int i = 0; i < N; ++i) u[i] = y0[i] * y0[i];
+#pragma unroll
+  for (int i = 0; i < N; ++i) e[i] = fma(-x[i], u[i], 1.0);
+#pragma unroll
+  for (int i = 0; i < N; ++i) u[i] = y0[i] * e[i];
+#pragma unroll
+  for (int i = 0; i < N; ++i) e[i] = fma(e[i], 0.375, 0.5);
+#pragma unroll
+  for (int i = 0; i < N; ++i) r[i] = fma(e[i], u[i], y0[i]);
+#pragma unroll
+  for (int i = 0; i < N; ++i) T[i][0] = cfar[i] * r[i];
+  if constexpr (L > 0) {
+    double h[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) h[i] = 0.5 * r[i];
+#pragma unroll
+    for (int i = 0; i < N; ++i) h[i] = h[i] * r[i];            // 1/(2x)
+#pragma unroll
+    for (int i = 0; i < N; ++i) T[i][1] = T[i][0] * h[i];
+#pragma unroll
+    for (int m = 1; m < L; ++m) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) T[i][m + 1] = T[i][m] * ((2 * m + 1) * h[i]);
+    }
+  }
+}
 template <int L>
 __device__ __forceinline__ void seeds_near(double x, double pref, const double* __restrict__ tab, double (&T)[L + 1]) {
   const double tm = fma(x, 16.0, 6755399441055744.0);
@@ -321,97 +356,72 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
                                                  const double (&gz)[NP], const double* __restrict__ boys_tab,
                                                  double (&acc)[NP][nlev(LA, LA + LB)]) {
   constexpr int L = LA + LB;
-  // KP primitive pairs are advanced together (independent dependency chains: the FP64 pipe has an 8-cycle latency and
-  // one warp's recurrence is a serial chain); the far-field vote is taken once for the group.
-  constexpr int KP = (WARP && L <= 1) ? 2 : 1;
+  // KP primitive pairs are advanced together: with the NP points that is KP*NP independent dependency chains per thread
+  // (the FP64 pipe has an 8-cycle latency, a warp issues in order); the far-field vote is taken once for the group.
+  constexpr int KP = (WARP && L <= 1 && NP <= 2) ? 2 : 1;
 #pragma unroll
   for (int s = 0; s < NP; ++s)
 #pragma unroll
     for (int i = 0; i < nlev(LA, L); ++i) acc[s][i] = 0.0;
 
   auto step = [&](auto kpc, int k) {
-    constexpr int K = decltype(kpc)::value;
+    constexpr int K = decltype(kpc)::value, N = K * NP;
     double2 q0[K], q1[K], q2[K];
-    double PCx[K][NP], PCy[K][NP], PCz[K][NP], x[K][NP], th0[K][NP][L + 1];
-    bool far = true;
+    double PCx[N], PCy[N], PCz[N], x[N], th0[N][L + 1];
 #pragma unroll
     for (int j = 0; j < K; ++j) {
       const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k + j);
       q0[j] = q[0]; q1[j] = q[1]; q2[j] = q[2];     // (p, inv2p) (Px, Py) (Pz, PAx)
-#pragma unroll
-      for (int s = 0; s < NP; ++s) {
-        PCx[j][s] = q1[j].x - gx[s]; PCy[j][s] = q1[j].y - gy[s]; PCz[j][s] = q2[j].x - gz[s];
-        x[j][s] = q0[j].x * fma(PCx[j][s], PCx[j][s], fma(PCy[j][s], PCy[j][s], PCz[j][s] * PCz[j][s]));
-        far = far && x[j][s] >= boys_xmax(L);
-      }
     }
+#pragma unroll
+    for (int j = 0; j < K; ++j)
+#pragma unroll
+      for (int s = 0; s < NP; ++s) { PCx[j * NP + s] = q1[j].x - gx[s]; PCy[j * NP + s] = q1[j].y - gy[s]; PCz[j * NP + s] = q2[j].x - gz[s]; }
+#pragma unroll
+    for (int i = 0; i < N; ++i) x[i] = PCz[i] * PCz[i];
+#pragma unroll
+    for (int i = 0; i < N; ++i) x[i] = fma(PCy[i], PCy[i], x[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) x[i] = fma(PCx[i], PCx[i], x[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) x[i] *= q0[i / NP].x;
+    bool far = true;
+#pragma unroll
+    for (int i = 0; i < N; ++i) far = far && x[i] >= boys_xmax(L);
     bool allfar = false;
     if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
     double2 q4[K];                                    // (pref, cfar)
 #pragma unroll
     for (int j = 0; j < K; ++j) q4[j] = reinterpret_cast<const double2*>(pp + k + j)[4];
     if (allfar) {
+      double cf[N];
 #pragma unroll
-      for (int j = 0; j < K; ++j)
-#pragma unroll
-        for (int s = 0; s < NP; ++s) seeds_far<L>(x[j][s], q4[j].y, th0[j][s]);
+      for (int i = 0; i < N; ++i) cf[i] = q4[i / NP].y;
+      seeds_far_v<L, N>(x, cf, th0);
     } else {
 #pragma unroll
-      for (int j = 0; j < K; ++j)
-#pragma unroll
-        for (int s = 0; s < NP; ++s) seeds<L>(x[j][s], q4[j].x, q4[j].y, boys_tab, th0[j][s]);
+      for (int i = 0; i < N; ++i) seeds<L>(x[i], q4[i / NP].x, q4[i / NP].y, boys_tab, th0[i]);
     }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
       if constexpr (L == 0) {
 #pragma unroll
-        for (int s = 0; s < NP; ++s) acc[s][0] += th0[j][s][0];
+        for (int s = 0; s < NP; ++s) acc[s][0] += th0[j * NP + s][0];
       } else {
         const double2 q3 = reinterpret_cast<const double2*>(pp + k + j)[3];   // (PAy, PAz)
 #pragma unroll
         for (int s = 0; s < NP; ++s)
-          vrr_accumulate<LA, L>(th0[j][s], q2[j].y, q3.x, q3.y, PCx[j][s], PCy[j][s], PCz[j][s], q0[j].y, acc[s]);
+          vrr_accumulate<LA, L>(th0[j * NP + s], q2[j].y, q3.x, q3.y, PCx[j * NP + s], PCy[j * NP + s], PCz[j * NP + s], q0[j].y, acc[s]);
       }
     }
   };
+  int k = 0;
   if constexpr (KP > 1) {
-    int k = 0;
 #pragma unroll 1
     for (; k + KP <= nprim; k += KP) step(std::integral_constant<int, KP>{}, k);
-#pragma unroll 1
-    for (; k < nprim; ++k) step(std::integral_constant<int, 1>{}, k);
-  } else {
-    for (int k = 0; k < nprim; ++k) {
-      const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k);
-      const double2 q0 = q[0], q1 = q[1], q2 = q[2];   // (p, inv2p) (Px, Py) (Pz, PAx)
-      double PCx[NP], PCy[NP], PCz[NP], x[NP], th0[NP][L + 1];
-      bool far = true;
-#pragma unroll
-      for (int s = 0; s < NP; ++s) {
-        PCx[s] = q1.x - gx[s]; PCy[s] = q1.y - gy[s]; PCz[s] = q2.x - gz[s];
-        x[s] = q0.x * fma(PCx[s], PCx[s], fma(PCy[s], PCy[s], PCz[s] * PCz[s]));
-        far = far && x[s] >= boys_xmax(L);
-      }
-      bool allfar = false;
-      if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
-      const double2 q4 = q[4];                          // (pref, cfar)
-      if (allfar) {
-#pragma unroll
-        for (int s = 0; s < NP; ++s) seeds_far<L>(x[s], q4.y, th0[s]);
-      } else {
-#pragma unroll
-        for (int s = 0; s < NP; ++s) seeds<L>(x[s], q4.x, q4.y, boys_tab, th0[s]);
-      }
-      if constexpr (L == 0) {
-#pragma unroll
-        for (int s = 0; s < NP; ++s) acc[s][0] += th0[s][0];
-      } else {
-        const double2 q3 = q[3];                        // (PAy, PAz)
-#pragma unroll
-        for (int s = 0; s < NP; ++s) vrr_accumulate<LA, L>(th0[s], q2.y, q3.x, q3.y, PCx[s], PCy[s], PCz[s], q0.y, acc[s]);
-      }
-    }
   }
+#pragma unroll 1
+  for (; k < nprim; ++k) step(std::integral_constant<int, 1>{}, k);
 }
 
 }  // namespace snk
