@@ -19,7 +19,7 @@ using namespace snk;
 namespace {
 thread_local std::string g_create_error;
 
-struct Super { int b0, b1; int64_t slot0, nslots; int t0, t1; };
+struct Super { int b0, b1; int64_t slot0, nslots; int t0, t1; int64_t f0; };   // f0: first 128-column tile (a4 activity bits)
 
 enum Stage { ST_SCREEN = 0, ST_COLLOC, ST_F, ST_G, ST_KT, ST_SYM, ST_COUNT };
 }  // namespace
@@ -45,6 +45,10 @@ struct snk_ctx {
   DevBuf<uint32_t> d_bmask;
   DevBuf<unsigned long long> d_phimax, d_Fmax;
   DevBuf<TileRec> d_tiles;
+  DevBuf<uint32_t> d_act;       // a6: activity bits of Phi blocks (row tile x 16-slot k-tile)
+  int64_t actw = 0;
+  DevBuf<uint32_t> d_actF;      // a4: activity bits of Phi blocks (128-slot column tile x 16-function k-tile)
+  int kwordsF = 0;
   std::vector<int32_t> h_bn;
   std::vector<int64_t> h_bslot;
   std::vector<TileRec> h_tiles;
@@ -63,6 +67,7 @@ struct snk_ctx {
   int64_t nprimpair = 0;
   int cls_beg[kNumClasses + 1] = {0};
   double gemm_flops = 0.0;
+  double flops_F = 0.0, flops_Kt = 0.0;     // a4 / a6 flops actually executed per build (blocks with a set activity bit)
   int64_t n_launches = 0;
   // timing
   std::vector<cudaEvent_t> ev_pool;
@@ -233,7 +238,7 @@ void snk_destroy(snk_ctx* ctx) {
   ctx->d_poff.release(); ctx->d_nprim.release(); ctx->d_lshells.release();
   ctx->gx.release(); ctx->gy.release(); ctx->gz.release(); ctx->gw.release(); ctx->d_PhiTf.release(); ctx->d_phit.release();
   ctx->slot_src.release(); ctx->d_bslot.release(); ctx->d_bn.release(); ctx->d_bmask.release(); ctx->d_phimax.release();
-  ctx->d_Fmax.release(); ctx->d_tiles.release(); ctx->d_Phi.release(); ctx->d_F.release(); ctx->d_G.release();
+  ctx->d_Fmax.release(); ctx->d_tiles.release(); ctx->d_act.release(); ctx->d_actF.release(); ctx->d_Phi.release(); ctx->d_F.release(); ctx->d_G.release();
   ctx->d_absP.release(); ctx->d_Ftf.release(); ctx->d_FtsT.release(); ctx->d_Kt.release();
   ctx->d_Pin.release(); ctx->d_Kout.release(); ctx->d_stats.release(); ctx->d_cflops.release();
   ctx->d_flag.release(); ctx->d_np.release(); ctx->d_pos.release(); ctx->d_ppos.release(); ctx->d_units.release();
@@ -442,6 +447,21 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       CK(ctx->gx.reserve(slot)); CK(ctx->gy.reserve(slot)); CK(ctx->gz.reserve(slot)); CK(ctx->gw.reserve(slot)); CK(ctx->slot_src.reserve(slot));
       CK(run_fill_slots(nb, d_bsrc_begin.p, ctx->d_bn.p, ctx->d_bslot.p, idx2.p, points, weights, ctx->gx.p, ctx->gy.p, ctx->gz.p,
                         ctx->gw.p, ctx->slot_src.p, s));
+      ctx->actw = (slot / 16 + 31) / 32 + 1;
+      CK(ctx->d_act.reserve((size_t)((ctx->nbf + 63) / 64) * ctx->actw));
+      CK(run_kt_flags(ctx->tab(), nb, ctx->d_bn.p, ctx->d_bslot.p, ctx->d_bmask.p, ctx->nshw, ctx->d_act.p, ctx->actw, s));
+      {   // executed a6 flops: 2 * rows of the tile * 16 * nbf per set bit
+        const int nmt = (ctx->nbf + 63) / 64;
+        std::vector<uint32_t> ha((size_t)nmt * ctx->actw);
+        CK(cudaMemcpyAsync(ha.data(), ctx->d_act.p, ha.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        ctx->flops_Kt = 0.0;
+        for (int mt = 0; mt < nmt; ++mt) {
+          int64_t bits = 0;
+          for (int64_t i = 0; i < ctx->actw; ++i) bits += __builtin_popcount(ha[(size_t)mt * ctx->actw + i]);
+          ctx->flops_Kt += 2.0 * std::min(64, ctx->nbf - 64 * mt) * 16.0 * ctx->nbf * (double)bits;
+        }
+      }
       // ---- Eq. 47 maxima (density independent) ----
       ctx->ldj = (nb + 7) / 8 * 8;
       CK(ctx->d_PhiTf.reserve((size_t)ctx->nbf * ctx->ldj)); CK(ctx->d_phit.reserve(nb));
@@ -477,6 +497,37 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
         }
         sp.b1 = j; sp.nslots = n; sp.t1 = t;
         ctx->supers.push_back(sp);
+      }
+      {   // a4 activity bits (density independent)
+        std::vector<int64_t> h_bslot0(nb), h_btile0(nb);
+        int64_t f = 0;
+        for (Super& sp : ctx->supers) {
+          sp.f0 = f;
+          for (int j = sp.b0; j < sp.b1; ++j) { h_bslot0[j] = sp.slot0; h_btile0[j] = f; }
+          f += (sp.nslots + 127) / 128;
+        }
+        ctx->kwordsF = ((ctx->nbf + 15) / 16 + 31) / 32;
+        DevBuf<int64_t> d_bslot0, d_btile0;
+        CK(upload(d_bslot0, h_bslot0)); CK(upload(d_btile0, h_btile0));
+        CK(ctx->d_actF.reserve((size_t)f * ctx->kwordsF));
+        CK(run_f_flags(ctx->tab(), nb, ctx->d_bn.p, ctx->d_bslot.p, d_bslot0.p, d_btile0.p, ctx->d_bmask.p, ctx->nshw, ctx->d_actF.p, f,
+                       ctx->kwordsF, s));
+        {   // executed a4 flops: 2 * nbf * (functions of the k-tile) * (columns of the tile) per set bit
+          std::vector<uint32_t> hf((size_t)f * ctx->kwordsF);
+          CK(cudaMemcpyAsync(hf.data(), ctx->d_actF.p, hf.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+          CK(cudaStreamSynchronize(s));
+          ctx->flops_F = 0.0;
+          const int nkt = (ctx->nbf + 15) / 16;
+          for (const Super& sp : ctx->supers) {
+            const int64_t nt = (sp.nslots + 127) / 128;
+            for (int64_t tt = 0; tt < nt; ++tt) {
+              const double cw = (double)std::min<int64_t>(128, sp.nslots - 128 * tt);
+              for (int kt = 0; kt < nkt; ++kt)
+                if ((hf[(size_t)(sp.f0 + tt) * ctx->kwordsF + (kt >> 5)] >> (kt & 31)) & 1u)
+                  ctx->flops_F += 2.0 * ctx->nbf * std::min(16, ctx->nbf - 16 * kt) * cw;
+            }
+          }
+        }
       }
       int64_t ld = 0;
       for (const Super& sp : ctx->supers) ld = std::max(ld, sp.nslots);
@@ -568,8 +619,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     span_end(sp);
     // ---- a4: F = P * Phi ----
     sp = span_begin(ST_F, -1);
-    CK(gemm_f64(false, nbf, su.nslots, nbf, P, nbf, ctx->d_Phi.p, ctx->ld, ctx->d_F.p, ctx->ld, false, nullptr, s));
-    ctx->gemm_flops += 2.0 * nbf * (double)su.nslots * nbf;
+    CK(gemm_f(nbf, su.nslots, P, ctx->d_Phi.p, ctx->d_F.p, ctx->ld, ctx->d_actF.p + su.f0 * ctx->kwordsF, ctx->kwordsF, s));
     span_end(sp);
     // ---- a5: G ----
     sp = span_begin(ST_G, -1);
@@ -589,11 +639,11 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     span_end(sp);
     // ---- a6: Kt += Phi diag(w) G^T ----
     sp = span_begin(ST_KT, -1);
-    CK(gemm_f64(true, nbf, nbf, su.nslots, ctx->d_Phi.p, ctx->ld, ctx->d_G.p, ctx->ld, ctx->d_Kt.p, nbf, true, ctx->gw.p + su.slot0, s));
-    ctx->gemm_flops += 2.0 * nbf * (double)su.nslots * nbf;
+    CK(gemm_kt(nbf, su.slot0, su.nslots, ctx->d_Phi.p, ctx->d_G.p, ctx->ld, ctx->gw.p, ctx->d_Kt.p, ctx->d_act.p, ctx->actw, s));
     ctx->n_launches += 3;   // collocation, F GEMM, Kt GEMM
     span_end(sp);
   }
+  ctx->gemm_flops += ctx->flops_F + ctx->flops_Kt;
   // ---- a7 ----
   sp = span_begin(ST_SYM, -1);
   CK(run_symmetrise(nbf, ctx->d_Kt.p, K, s));
