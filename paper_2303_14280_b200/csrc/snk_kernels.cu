@@ -144,8 +144,8 @@ __global__ void k_bbox(const int64_t* __restrict__ begin, const uint32_t* __rest
 // a1: shell a in B_j iff dist^2(A, bbox_j) <= rcut_a^2 (R10).  mode 0: count shells per batch; mode 1: bit masks.
 __global__ void k_basis_screen(ShellTab sh, const double* __restrict__ bbox, const int32_t* __restrict__ batch_src, int nbatch, int nshw,
                                int32_t* __restrict__ count, uint32_t* __restrict__ mask) {
-  const int j = blockIdx.y;
-  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.x;                      // batches on grid.x: more than 65535 of them at the paper's scale
+  const int a = blockIdx.y * blockDim.x + threadIdx.x;
   const double* bb = bbox + 6 * (int64_t)(batch_src ? batch_src[j] : j);
   bool in = false;
   if (a < sh.nsh) {
@@ -374,8 +374,8 @@ __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict_
 // V_j bit masks (Eq. 43): one thread per (batch, unit); every unit of a pair takes the pair's decision
 __global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const double* __restrict__ FtsT, int nshld,
                         const double* __restrict__ phit, double eps, uint32_t* __restrict__ vmask, int64_t vstride) {
-  const int j = blockIdx.y;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.x;
+  const int i = blockIdx.y * blockDim.x + threadIdx.x;
   bool keep = false;
   if (i < nunit) {
     const UnitMeta m = meta[i];
@@ -394,8 +394,8 @@ __global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const doub
 __global__ void k_vstats(int nunit, const UnitMeta* __restrict__ meta, ShellTab sh, const int32_t* __restrict__ bn,
                          const uint32_t* __restrict__ vmask, int64_t vstride, const double* __restrict__ class_flops_prim,
                          const double* __restrict__ class_flops_contr, double* __restrict__ out) {
-  const int j = blockIdx.y;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.x;
+  const int i = blockIdx.y * blockDim.x + threadIdx.x;
   if (i >= nunit) return;
   if (!((vmask[(int64_t)j * vstride + (i >> 5)] >> (i & 31)) & 1u)) return;
   const UnitMeta m = meta[i];
@@ -515,7 +515,7 @@ cudaError_t run_bbox(int nbatch, const int64_t* begin, const uint32_t* idx, cons
 cudaError_t run_basis_screen(const ShellTab& sh, const double* bbox, const int32_t* batch_src, int nbatch, int nshw, int32_t* count,
                              uint32_t* mask, cudaStream_t s) {
   if (nbatch > 0) {
-    dim3 g((unsigned)(nshw * 32 + 127) / 128, (unsigned)nbatch);
+    dim3 g((unsigned)nbatch, (unsigned)(nshw * 32 + 127) / 128);
     k_basis_screen<<<g, 128, 0, s>>>(sh, bbox, batch_src, nbatch, nshw, count, mask);
   }
   return cudaGetLastError();
@@ -571,7 +571,7 @@ cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t*
 cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
                       uint32_t* vmask, int64_t vstride, cudaStream_t s) {
   if (nbatch > 0 && nunit > 0) {
-    dim3 g(nblk(nunit, 256), (unsigned)nbatch);
+    dim3 g((unsigned)nbatch, nblk(nunit, 256));
     k_vmask<<<g, 256, 0, s>>>(nunit, meta, FtsT, nshld, phit, eps, vmask, vstride);
   }
   return cudaGetLastError();
@@ -580,7 +580,7 @@ cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double*
 cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
                        int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s) {
   if (nbatch > 0 && nunit > 0) {
-    dim3 g(nblk(nunit, 256), (unsigned)nbatch);
+    dim3 g((unsigned)nbatch, nblk(nunit, 256));
     k_vstats<<<g, 256, 0, s>>>(nunit, meta, sh, bn, vmask, vstride, cfp, cfc, out);
   }
   return cudaGetLastError();

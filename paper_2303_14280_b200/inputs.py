@@ -178,7 +178,7 @@ def make_basis(rng: np.random.Generator, zs: np.ndarray, xyz_bohr: np.ndarray, s
 
 
 def becke_grid(xyz_bohr: np.ndarray, n_r: int, n_theta: int, n_phi: int, *, partner_cut_ang: float = 10.0,
-               w_min: float = 1e-15, device: str = "cpu", chunk_bytes: int = 1 << 28):
+               w_min: float = 1e-15, device: str = "cpu", chunk_bytes: int = 1 << 28, parents=None):
     """Product atomic grids + Becke partition (stands in for the
     paper's MK x Lebedev / SSF grid).
 
@@ -189,6 +189,8 @@ def becke_grid(xyz_bohr: np.ndarray, n_r: int, n_theta: int, n_phi: int, *, part
     Becke: w <- w * p_A / sum_B p_B, p_A = prod_{B != A} s(mu_AB), s = (1 - f(f(f(mu))))/2,
            f = 1.5 mu - 0.5 mu^3; partners restricted to atoms within ``partner_cut_ang`` Å of the parent.
     Points with weight < w_min are dropped.  Order: atom, radial, theta, phi (phi fastest).
+    ``parents``: generate only the atomic grids of these atoms (their points and weights are exactly those of the full
+    molecular grid, the partition still sees every partner); tests use it to cut a piece out of a large config.
     Returns (points [n,3], weights [n]) as numpy float64.
     """
     import torch
@@ -217,7 +219,7 @@ def becke_grid(xyz_bohr: np.ndarray, n_r: int, n_theta: int, n_phi: int, *, part
     dist_aa = torch.cdist(xyz, xyz)
     cut = partner_cut_ang * BOHR_PER_ANGSTROM
     pts_out, w_out = [], []
-    for A in range(nat):
+    for A in (range(nat) if parents is None else [int(a) for a in parents]):
         nb = torch.nonzero(dist_aa[A] <= cut).reshape(-1)              # includes A itself
         nn = int(nb.numel())
         pts = local + xyz[A]
@@ -254,10 +256,11 @@ def density_from_C(rng: np.random.Generator, nbf: int, nocc: int, sigma: float) 
     return 0.5 * (P + P.T)
 
 
-def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, natoms=None) -> Workload:
+def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, natoms=None, grid_atoms=None) -> Workload:
     """BASELINE.json config ``cfg`` (1..5).  ``grid=(n_r,n_theta,n_phi)`` overrides the grid level
     (reduced levels are what the CPU-sized parity tests use); ``lattice`` / ``natoms`` shrink
-    the molecule (tests only).  Everything else (seed, draw order) is fixed."""
+    the molecule (tests only); ``grid_atoms`` keeps the whole molecule, basis and P but only the atomic grids of the
+    listed atoms (tests only).  Everything else (seed, draw order) is fixed."""
     c = CONFIGS[cfg]
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + cfg))
     # draw order: geometry -> basis -> C
@@ -277,7 +280,7 @@ def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, nat
     sigma = c["sigma"] if c["sigma"] is not None else 1.0 / math.sqrt(nocc)
     P = density_from_C(rng, nbf, nocc, sigma)
     g = grid or c["grid"]
-    pts, w = becke_grid(xyz, *g, device=device)
+    pts, w = becke_grid(xyz, *g, device=device, parents=grid_atoms)
     return Workload(name=c["name"], cfg=cfg, basis=basis, points=pts, weights=w, P=P, eps=c["eps"],
                     grid_shape=tuple(g), atoms_z=tuple(int(z) for z in zs))
 

@@ -252,3 +252,14 @@ def test_K_cfg3_full_size_sampled(snk_mod, oracle_mod, torch_cuda):
 def test_K_cfg5_full_size_sampled(snk_mod, oracle_mod, torch_cuda):
     """configs[4] (32 atoms with s..f shells, 992 functions, 1.24M points, eps 1e-12) at full size: all ten classes."""
     _full_size_sampled(snk_mod, oracle_mod, torch_cuda, 5, 0.004, "cfg5-full", scale_abs=True)
+
+
+def test_K_cfg4_subgrid(snk_mod, oracle_mod):
+    """configs[3] (343 waters, 8575 functions, eps 1e-10): the whole molecule, basis and density, on a piece of its grid the
+    oracle can afford -- 1500 seeded points out of the atomic grids of one central water (about 3.3e6 contracted integrals per
+    point: every significant pair survives the screening with this density).  Same points to both sides, lists audited."""
+    w = inputs.make_workload(4, grid_atoms=[513, 514, 515], device="cuda")
+    rng = np.random.Generator(np.random.PCG64(inputs.SEED_BASE + 44))
+    sel = np.sort(rng.choice(w.points.shape[0], size=1500, replace=False))
+    w.points, w.weights = np.ascontiguousarray(w.points[sel]), np.ascontiguousarray(w.weights[sel])
+    _run_both(snk_mod, oracle_mod, w, batch_max=256, tag="cfg4-subgrid")
