@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <string>
@@ -564,6 +565,13 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     ctx->npair_sig = 0; ctx->nunit = 0; ctx->nprimpair = 0; ctx->have_build = true;
     return SNK_OK;
   }
+  // SNK_TRACE=1: synchronise after every stage and report it on stderr (debugging aid; perturbs the timings)
+  static const bool trace = getenv("SNK_TRACE") != nullptr;
+  auto tr = [&](const char* what, int a, int b) {
+    if (!trace) return;
+    const cudaError_t e = cudaStreamSynchronize(s);
+    fprintf(stderr, "[snk] %s %d/%d: %s\n", what, a, b, cudaGetErrorString(e));
+  };
   auto span_begin = [&](int stage, int cls) { snk_ctx::Span sp{stage, cls, ctx->new_event(), -1}; cudaEventRecord(ctx->ev_pool[sp.e0], s); return sp; };
   auto span_end = [&](snk_ctx::Span sp) { sp.e1 = ctx->new_event(); cudaEventRecord(ctx->ev_pool[sp.e1], s); ctx->spans.push_back(sp); };
 
@@ -608,6 +616,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   CK(run_vmask(nb, nunit, ctx->d_meta.p, ctx->d_FtsT.p, nsh, ctx->d_phit.p, ctx->eps, ctx->d_vmask.p, ctx->vstride, s));
   ctx->n_launches += 6;
   span_end(sp);
+  tr("screen", nunit, npair);
 
   CK(cudaMemsetAsync(ctx->d_Kt.p, 0, (size_t)nbf * nbf * sizeof(double), s));
   for (const Super& su : ctx->supers) {
@@ -619,8 +628,10 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     span_end(sp);
     // ---- a4: F = P * Phi ----
     sp = span_begin(ST_F, -1);
+    tr("colloc", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
     CK(gemm_f(nbf, su.nslots, P, ctx->d_Phi.p, ctx->d_F.p, ctx->ld, ctx->d_actF.p + su.f0 * ctx->kwordsF, ctx->kwordsF, s));
     span_end(sp);
+    tr("F", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
     // ---- a5: G ----
     sp = span_begin(ST_G, -1);
     CK(cudaMemsetAsync(ctx->d_G.p, 0, (size_t)nbf * ctx->ld * sizeof(double), s));
@@ -635,6 +646,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
       CK(launch_integrals(c, ip, s));
       ctx->n_launches += 1;
       span_end(spc);
+      tr("G class", c, kNumClasses);
     }
     span_end(sp);
     // ---- a6: Kt += Phi diag(w) G^T ----
@@ -642,6 +654,7 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     CK(gemm_kt(nbf, su.slot0, su.nslots, ctx->d_Phi.p, ctx->d_G.p, ctx->ld, ctx->gw.p, ctx->d_Kt.p, ctx->d_act.p, ctx->actw, s));
     ctx->n_launches += 3;   // collocation, F GEMM, Kt GEMM
     span_end(sp);
+    tr("Kt", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
   }
   ctx->gemm_flops += ctx->flops_F + ctx->flops_Kt;
   // ---- a7 ----
