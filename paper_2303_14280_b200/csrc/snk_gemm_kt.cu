@@ -6,7 +6,7 @@
 //   * Operand tiles travel global -> shared with 16-byte cp.async in a 4-stage ring (one __syncthreads per k-tile); the
 //     shared rows keep the k-contiguous order with a row stride of 20 doubles, which makes the fragment loads
 //     (thread (g,t) reads [row g][k t]) hit 16 distinct 8-byte banks per half warp.
-//   * w_g is staged with the tile and folded into the G fragments.
+//   * w_g is staged with the tile and folded into the Phi fragments.
 //   * Basis screening (Eq. 41): Phi rows of shells outside B_j are identically zero over batch j.  A bit per
 //     (64-function row tile, 16-slot k-tile) says whether any function of the row tile is in B_j of the batch that owns
 //     the k-tile; the kernel walks only the set bits (batches start on 32-slot boundaries, so a k-tile never straddles
