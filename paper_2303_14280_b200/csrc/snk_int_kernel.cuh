@@ -3,13 +3,13 @@
 // up to kTile consecutive points of one batch.  A is never stored.
 //
 // B200 design (differs from the paper's A100 kernel):
-//   * warp-specialised: warps 0..3 are consumers, warp 4 is a producer that walks the tile's V_j bit mask and streams
+//   * warp-specialised: warps 0..CW-1 are consumers (CW = 8 for L <= 2, else 4), warp CW is a producer that walks the tile's V_j bit mask and streams
 //     every kept pair unit -- header + primitive pairs (<= 704 B) and the F_b rows of this tile -- into a ring of
 //     shared-memory slots with cp.async.bulk (TMA bulk copy) completing on an mbarrier; consumers never touch pair
 //     data in global memory, so the recurrences run against broadcast LDS only;
-//   * a consumer thread owns NP points of the tile (4 for L <= 1, 2 for L = 2, else 1) and the NP warps that cover the
-//     same points split the unit stream dynamically (shared-memory ticket): the point-independent work of a unit is
-//     paid once per 32 NP points;
+//   * a consumer thread owns NP points of the tile (2 for L <= 1, else 1) and the warps that cover the same points
+//     (4 of the 8 consumer warps for L <= 1, 2 for L = 2) split the unit stream dynamically (shared-memory ticket): the
+//     point-independent work of a unit is paid once per 32 NP points and one staged unit feeds more resident chains;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
 //     fire-and-forget RED.F64 (coalesced along the slot index);
 //   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh).
@@ -26,13 +26,13 @@ namespace snk {
 // NP recurrences are independent instruction streams.  The tile is therefore covered by G = 4 / NP point groups of NP warps
 // each, and the warps of one group share the unit stream: each takes the next unit nobody of its group has taken yet.
 #ifndef SNK_NP_L0
-#define SNK_NP_L0 4
+#define SNK_NP_L0 2
 #endif
 #ifndef SNK_NP_L1
-#define SNK_NP_L1 4
+#define SNK_NP_L1 2
 #endif
 #ifndef SNK_NP_L2
-#define SNK_NP_L2 2
+#define SNK_NP_L2 1
 #endif
 #ifndef SNK_NP_L3
 #define SNK_NP_L3 1
@@ -43,13 +43,13 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
 }
 // resident CTAs per SM the register allocation is held to
 #ifndef SNK_MB_L0
-#define SNK_MB_L0 4
+#define SNK_MB_L0 3
 #endif
 #ifndef SNK_MB_L1
-#define SNK_MB_L1 3
+#define SNK_MB_L1 2
 #endif
 #ifndef SNK_MB_L2
-#define SNK_MB_L2 3
+#define SNK_MB_L2 2
 #endif
 #ifndef SNK_MB_L3
 #define SNK_MB_L3 3
@@ -58,7 +58,25 @@ __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
   const int L = LA + LB;
   return L == 0 ? SNK_MB_L0 : L == 1 ? SNK_MB_L1 : L == 2 ? SNK_MB_L2 : L == 3 ? SNK_MB_L3 : L == 4 ? 2 : 1;
 }
-__host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile + 32; }
+// consumer warps per CTA: NP per point group by default; more (SNK_CW_L*) let a group's unit stream be shared by more
+// warps, i.e. more resident point chains per staged unit and per producer warp
+#ifndef SNK_CW_L0
+#define SNK_CW_L0 8
+#endif
+#ifndef SNK_CW_L1
+#define SNK_CW_L1 8
+#endif
+#ifndef SNK_CW_L2
+#define SNK_CW_L2 8
+#endif
+#ifndef SNK_CW_L3
+#define SNK_CW_L3 4
+#endif
+__host__ __device__ constexpr int int_cw(int LA, int LB) {
+  const int L = LA + LB;
+  return L == 0 ? SNK_CW_L0 : L == 1 ? SNK_CW_L1 : L == 2 ? SNK_CW_L2 : L == 3 ? SNK_CW_L3 : 4;
+}
+__host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_cw(LA, LB) + 32; }
 
 #ifndef SNK_NS_LB0
 #define SNK_NS_LB0 8
@@ -66,7 +84,7 @@ __host__ __device__ constexpr int int_threads(int LA, int LB) { return kTile + 3
 #ifndef SNK_NS_LB1
 #define SNK_NS_LB1 8
 #endif
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8; }
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return (LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8) * (int_cw(LA, LB) / 4); }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
 // ring slots, then full[NS] and empty[NS] mbarriers, then the per-group unit counters and the unit count
 __host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB) + 32; }
@@ -226,7 +244,9 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 template <int LA, int LB>
 __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_integrals(IntParams p) {
   constexpr int NB = ncart(LB);
-  constexpr int NPM = int_npmax(LA, LB), CW = kTile / 32;           // points per thread, consumer warps per CTA
+  constexpr int NPM = int_npmax(LA, LB), CW = int_cw(LA, LB);       // points per thread, consumer warps per CTA
+  constexpr int WPG = CW * NPM * 32 / kTile;                         // consumer warps per point group
+  static_assert(CW % 4 == 0 && WPG >= 1, "consumer warps");
   constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
@@ -299,7 +319,7 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
     }
     return;
   }
-  const int grp = warp / NPM, pbase = grp * 32 * NPM;
+  const int grp = warp / WPG, pbase = grp * 32 * NPM;
   if (pbase >= tile.n) return;
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
   int* s_next = s_ctr + grp;

@@ -352,7 +352,7 @@ struct StoreSink {
 // WARP: all 32 lanes call together; when every point of the warp is in the far field of a primitive pair (the common
 // case in the paper-shaped workloads) the Boys function runs without table loads or branches.
 #ifndef SNK_KP2_MAXNP
-#define SNK_KP2_MAXNP 2
+#define SNK_KP2_MAXNP 1
 #endif
 template <int LA, int LB, int NP, bool WARP>
 __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp, int nprim, const double (&gx)[NP], const double (&gy)[NP],
