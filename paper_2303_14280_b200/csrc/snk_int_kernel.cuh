@@ -84,7 +84,7 @@ __host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_
 #ifndef SNK_NS_LB1
 #define SNK_NS_LB1 8
 #endif
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return (LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8) * (int_cw(LA, LB) / 4); }
+__host__ __device__ constexpr int int_nslots(int LA, int LB) { return (LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8) * int_cw(LA, LB) / 4; }
 __host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
 // ring slots, then full[NS] and empty[NS] mbarriers, then the per-group unit counters and the unit count
 __host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB) + 32; }
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   constexpr int NB = ncart(LB);
   constexpr int NPM = int_npmax(LA, LB), CW = int_cw(LA, LB);       // points per thread, consumer warps per CTA
   constexpr int WPG = CW * NPM * 32 / kTile;                         // consumer warps per point group
-  static_assert(CW % 4 == 0 && WPG >= 1, "consumer warps");
+  static_assert(WPG >= 1 && WPG * (kTile / (32 * NPM)) == CW, "consumer warps: a whole number per point group");
   constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
