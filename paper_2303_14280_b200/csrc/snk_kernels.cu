@@ -391,29 +391,55 @@ __global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const doub
 // counters for snk_stats: out[0]=sum|V_j|, [1]=pair-points, [2]=contracted integrals, [3]=primitive integrals,
 // [4..13] contracted integrals per class, [14] flop model, [16..25] flop model per class.  Pair-level quantities are
 // counted on the first unit of a pair only.
-__global__ void k_vstats(int nunit, const UnitMeta* __restrict__ meta, ShellTab sh, const int32_t* __restrict__ bn,
-                         const uint32_t* __restrict__ vmask, int64_t vstride, const double* __restrict__ class_flops_prim,
-                         const double* __restrict__ class_flops_contr, double* __restrict__ out) {
+// One CTA per batch walks the batch's V_j mask; sums are kept in registers, reduced over the CTA and leave with 23 atomics
+// per batch (one atomic per kept unit and counter would serialise 10^11 same-address updates at the paper's scale).
+__global__ void __launch_bounds__(256) k_vstats(int nunit, const UnitMeta* __restrict__ meta, ShellTab sh, const int32_t* __restrict__ bn,
+                                                const uint32_t* __restrict__ vmask, int64_t vstride,
+                                                const double* __restrict__ class_flops_prim, const double* __restrict__ class_flops_contr,
+                                                double* __restrict__ out) {
+  constexpr int NV = 3 + 2 * kNumClasses;
+  __shared__ double red[8][NV];
   const int j = blockIdx.x;
-  const int i = blockIdx.y * blockDim.x + threadIdx.x;
-  if (i >= nunit) return;
-  if (!((vmask[(int64_t)j * vstride + (i >> 5)] >> (i & 31)) & 1u)) return;
-  const UnitMeta m = meta[i];
-  const int la = sh.l[m.sa], lb = sh.l[m.sb];
-  const int np = m.nprim_first & 0xff;
-  const double first = (double)((m.nprim_first >> 8) & 1);
-  const double nq = bn[j], nc = (double)(ncart(la) * ncart(lb));
-  const int cls = la * (la + 1) / 2 + lb;
-  if (first > 0.0) {
-    atomicAdd(out + 0, 1.0);
-    atomicAdd(out + 1, nq);
-    atomicAdd(out + 2, nq * nc);
-    atomicAdd(out + 4 + cls, nq * nc);
+  const double nq = bn[j];
+  double v[NV];                                  // [0] kept pairs, [1] pair-points, [2] primitive integrals, then per class
+#pragma unroll
+  for (int k = 0; k < NV; ++k) v[k] = 0.0;
+  const uint32_t* __restrict__ mrow = vmask + (int64_t)j * vstride;
+  for (int i = threadIdx.x; i < nunit; i += 256) {
+    if (!((mrow[i >> 5] >> (i & 31)) & 1u)) continue;
+    const UnitMeta m = meta[i];
+    const int la = sh.l[m.sa], lb = sh.l[m.sb];
+    const int np = m.nprim_first & 0xff;
+    const double first = (double)((m.nprim_first >> 8) & 1);
+    const double nc = (double)(ncart(la) * ncart(lb));
+    const int cls = la * (la + 1) / 2 + lb;
+    v[0] += first; v[1] += first * nq; v[2] += nq * nc * np;
+    const double vi = first * nq * nc, vf = nq * (class_flops_prim[cls] * np + class_flops_contr[cls] * first);
+#pragma unroll
+    for (int c = 0; c < kNumClasses; ++c)
+      if (c == cls) { v[3 + c] += vi; v[3 + kNumClasses + c] += vf; }
   }
-  atomicAdd(out + 3, nq * nc * np);
-  const double fl = nq * (class_flops_prim[cls] * np + class_flops_contr[cls] * first);
-  atomicAdd(out + 14, fl);
-  atomicAdd(out + 16 + cls, fl);
+#pragma unroll
+  for (int k = 0; k < NV; ++k) {
+    double x = v[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5][k] = x;
+  }
+  __syncthreads();
+  if (threadIdx.x < NV) {
+    const int k = threadIdx.x;
+    double x = 0.0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) x += red[w][k];
+    if (x != 0.0) {
+      if (k == 0) atomicAdd(out + 0, x);
+      else if (k == 1) atomicAdd(out + 1, x);
+      else if (k == 2) atomicAdd(out + 3, x);
+      else if (k < 3 + kNumClasses) { atomicAdd(out + 4 + (k - 3), x); atomicAdd(out + 2, x); }
+      else { atomicAdd(out + 16 + (k - 3 - kNumClasses), x); atomicAdd(out + 14, x); }
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -580,8 +606,7 @@ cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double*
 cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
                        int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s) {
   if (nbatch > 0 && nunit > 0) {
-    dim3 g((unsigned)nbatch, nblk(nunit, 256));
-    k_vstats<<<g, 256, 0, s>>>(nunit, meta, sh, bn, vmask, vstride, cfp, cfc, out);
+    k_vstats<<<(unsigned)nbatch, 256, 0, s>>>(nunit, meta, sh, bn, vmask, vstride, cfp, cfc, out);
   }
   return cudaGetLastError();
 }
