@@ -449,10 +449,10 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       CK(run_fill_slots(nb, d_bsrc_begin.p, ctx->d_bn.p, ctx->d_bslot.p, idx2.p, points, weights, ctx->gx.p, ctx->gy.p, ctx->gz.p,
                         ctx->gw.p, ctx->slot_src.p, s));
       ctx->actw = (slot / 16 + 31) / 32 + 1;
-      CK(ctx->d_act.reserve((size_t)((ctx->nbf + 63) / 64) * ctx->actw));
+      CK(ctx->d_act.reserve((size_t)((ctx->nbf + kt_row_tile() - 1) / kt_row_tile()) * ctx->actw));
       CK(run_kt_flags(ctx->tab(), nb, ctx->d_bn.p, ctx->d_bslot.p, ctx->d_bmask.p, ctx->nshw, ctx->d_act.p, ctx->actw, s));
       {   // executed a6 flops: 2 * rows of the tile * 16 * nbf per set bit
-        const int nmt = (ctx->nbf + 63) / 64;
+        const int nmt = (ctx->nbf + kt_row_tile() - 1) / kt_row_tile();
         std::vector<uint32_t> ha((size_t)nmt * ctx->actw);
         CK(cudaMemcpyAsync(ha.data(), ctx->d_act.p, ha.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
         CK(cudaStreamSynchronize(s));
@@ -460,7 +460,7 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
         for (int mt = 0; mt < nmt; ++mt) {
           int64_t bits = 0;
           for (int64_t i = 0; i < ctx->actw; ++i) bits += __builtin_popcount(ha[(size_t)mt * ctx->actw + i]);
-          ctx->flops_Kt += 2.0 * std::min(64, ctx->nbf - 64 * mt) * 16.0 * ctx->nbf * (double)bits;
+          ctx->flops_Kt += 2.0 * std::min(kt_row_tile(), ctx->nbf - kt_row_tile() * mt) * 16.0 * ctx->nbf * (double)bits;
         }
       }
       // ---- Eq. 47 maxima (density independent) ----

@@ -1,14 +1,15 @@
 // snk_gemm_kt.cu -- a6:  Kt[mu,nu] += sum_g Phi[mu,g] w_g G[nu,g]        Eq. 39, fp64 DMMA (m8n8k4)
 //
 // Both operands are rows of the [nbf x ld] slabs of one super-batch, i.e. contiguous along the contraction index g.
-//   * CTA tile 64 (Phi rows) x 256 (G rows), k-tile 16 slots, 8 warps (2 x 4), warp tile 32 x 64 = 4 x 8 fragments,
-//     accumulators in registers.
+//   * CTA tile 32 (Phi rows) x 256 (G rows), k-tile 16 slots, 8 warps (1 x 8), warp tile 32 x 32 = 4 x 4 fragments,
+//     accumulators in registers.  (64 x 256 with 2 x 4 warps has the better operand reuse but skips fewer blocks:
+//     490 vs 427 ms on cfg 3.)
 //   * Operand tiles travel global -> shared with 16-byte cp.async in a 4-stage ring (one __syncthreads per k-tile); the
 //     shared rows keep the k-contiguous order with a row stride of 20 doubles, which makes the fragment loads
 //     (thread (g,t) reads [row g][k t]) hit 16 distinct 8-byte banks per half warp.
 //   * w_g is staged with the tile and folded into the Phi fragments.
 //   * Basis screening (Eq. 41): Phi rows of shells outside B_j are identically zero over batch j.  A bit per
-//     (64-function row tile, 16-slot k-tile) says whether any function of the row tile is in B_j of the batch that owns
+//     (32-function row tile, 16-slot k-tile) says whether any function of the row tile is in B_j of the batch that owns
 //     the k-tile; the kernel walks only the set bits (batches start on 32-slot boundaries, so a k-tile never straddles
 //     two batches).  Skipped tiles contribute exact zeros, so the result is unchanged.
 //   * split-K into short k-chunks (2048 slots) gives thousands of CTAs whatever nbf is; partial tiles are RED-added into Kt.
@@ -60,13 +61,17 @@ struct BitWalk {
 };
 
 // CTA tile TA (Phi rows) x TB (G rows): the Phi side is kept narrow because that is where the zero blocks are
-constexpr int TA = 64, TB = 256, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK, KT_STAGES = 4;
+#ifndef SNK_KT_TA
+#define SNK_KT_TA 32
+#endif
+constexpr int TA = SNK_KT_TA, TB = 256, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK, KT_STAGES = 4;
+constexpr int KT_WM = TA / 32, KT_WN = 8 / KT_WM, KT_NJ = TB / KT_WN / 8;   // warps along Phi rows / G rows, fragments per warp along G
 __global__ void __launch_bounds__(NTH) k_gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* __restrict__ Phi,
                                                  const double* __restrict__ G, int64_t ld, const double* __restrict__ wts,
                                                  double* __restrict__ Kt, const uint32_t* __restrict__ act, int64_t actw, int64_t wchunk) {
   extern __shared__ __align__(16) double smem_kt[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = warp >> 2, wn = warp & 3;                 // 2 x 4 warps, warp tile 32 x 64 = 4 x 8 fragments
+  const int wm = warp / KT_WN, wn = warp % KT_WN;          // KT_WM x KT_WN warps, warp tile 32 x (8 KT_NJ)
   const int g = lane >> 2, t = lane & 3;
   const int64_t m0 = (int64_t)blockIdx.y * TA, n0 = (int64_t)blockIdx.x * TB;
   const int64_t kt0 = slot0 / TK, kt1 = (slot0 + nslots) / TK;
@@ -95,11 +100,11 @@ __global__ void __launch_bounds__(NTH) k_gemm_kt(int64_t nbf, int64_t slot0, int
     if (tid < 8) cp_async16(sa + (uint32_t)((TA + TB) * LDK + tid * 2) * 8u, wts + ktg * TK + tid * 2, 16u);
   };
 
-  double acc[4][8][2];
+  double acc[4][KT_NJ][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    for (int j = 0; j < KT_NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
   int64_t pending = walk.next();                           // next k-tile to issue
   int issued = 0;
@@ -115,20 +120,20 @@ __global__ void __launch_bounds__(NTH) k_gemm_kt(int64_t nbf, int64_t slot0, int
     cp_commit();
     const double* st = smem_kt + (it % KT_STAGES) * KT_STAGE_DOUBLES;
     const double* as = st + (wm * 32 + g) * LDK + t;
-    const double* bs = st + TA * LDK + (wn * 64 + g) * LDK + t;
+    const double* bs = st + TA * LDK + (wn * 8 * KT_NJ + g) * LDK + t;
     const double* ws = st + (TA + TB) * LDK + t;
 #pragma unroll
     for (int kk = 0; kk < TK; kk += 4) {
-      double af[4], bf[8];
+      double af[4], bf[KT_NJ];
       const double wk = ws[kk];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = as[i * 8 * LDK + kk] * wk;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) bf[j] = bs[j * 8 * LDK + kk];
+      for (int j = 0; j < KT_NJ; ++j) bf[j] = bs[j * 8 * LDK + kk];
 #pragma unroll
       for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        for (int j = 0; j < KT_NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     }
   }
   if (issued == 0) return;
@@ -138,8 +143,8 @@ __global__ void __launch_bounds__(NTH) k_gemm_kt(int64_t nbf, int64_t slot0, int
     const int64_t row = m0 + wm * 32 + i * 8 + g;
     if (row >= nbf) continue;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const int64_t col = n0 + wn * 64 + j * 8 + 2 * t;
+    for (int j = 0; j < KT_NJ; ++j) {
+      const int64_t col = n0 + wn * 8 * KT_NJ + j * 8 + 2 * t;
       double* c = Kt + row * nbf + col;
       if (col < nbf) atomicAdd(c, acc[i][j][0]);
       if (col + 1 < nbf) atomicAdd(c + 1, acc[i][j][1]);
@@ -274,6 +279,8 @@ __global__ void __launch_bounds__(128) k_kt_flags(ShellTab sh, const int32_t* __
 }  // namespace snk
 
 namespace snk {
+
+int kt_row_tile() { return TA; }
 
 cudaError_t run_kt_flags(const ShellTab& sh, int nbatch, const int32_t* bn, const int64_t* bslot, const uint32_t* bmask, int nshw,
                          uint32_t* act, int64_t actw, cudaStream_t s) {

@@ -55,6 +55,7 @@ cudaError_t run_f_flags(const ShellTab& sh, int nbatch, const int32_t* bn, const
                         const int64_t* btile0, const uint32_t* bmask, int nshw, uint32_t* act, int64_t ntiles, int kwords, cudaStream_t s);
 cudaError_t gemm_f(int64_t nbf, int64_t ncols, const double* P, const double* Phi, double* F, int64_t ld, const uint32_t* act, int kwords,
                    cudaStream_t s);
+int kt_row_tile();   // Phi rows per CTA tile of k_gemm_kt = granularity of its activity bits
 cudaError_t gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* Phi, const double* G, int64_t ld, const double* wts,
                     double* Kt, const uint32_t* act, int64_t actw, cudaStream_t s);
 cudaError_t run_zero_pad_cols(double* A, int64_t rows, int64_t ld, int64_t c0, int64_t c1, cudaStream_t s);
