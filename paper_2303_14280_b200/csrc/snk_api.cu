@@ -371,6 +371,7 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
   ctx->h_bn.clear(); ctx->h_bslot.clear(); ctx->h_tiles.clear(); ctx->supers.clear();
   ctx->nshw = (nsh + 31) / 32;
   std::vector<int64_t> h_bsrc_begin;
+  std::vector<int32_t> h_bcnt;          // |B_j| of the kept batches
   std::vector<int32_t> h_bsrc;
   DevBuf<uint32_t> idx0, idx1, idx2;
   if (npts > 0) {
@@ -431,6 +432,7 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       h_bsrc.push_back(j); h_bsrc_begin.push_back(h_begin[j]);
       ctx->h_bn.push_back(n); ctx->h_bslot.push_back(slot);
       ctx->sum_B += h_cnt[j];
+      h_bcnt.push_back(h_cnt[j]);
       ctx->npts_kept += n;
       slot += (n + kSlotAlign - 1) / kSlotAlign * kSlotAlign;
     }
@@ -481,7 +483,6 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       for (int j = 0; j < nb; ++j)
         for (int o = 0; o < ctx->h_bn[j]; o += kTile)
           ctx->h_tiles.push_back(TileRec{j, std::min(kTile, ctx->h_bn[j] - o), ctx->h_bslot[j] + o});
-      CK(upload(ctx->d_tiles, ctx->h_tiles));
       const double budget = ctx->workspace_gb * 1073741824.0;
       int64_t max_slots = (int64_t)(budget / (3.0 * 8.0 * std::max(1, ctx->nbf)));
       max_slots = std::max<int64_t>(max_slots / 128 * 128, 4096 + kSlotAlign);
@@ -499,6 +500,13 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
         sp.b1 = j; sp.nslots = n; sp.t1 = t;
         ctx->supers.push_back(sp);
       }
+      // The CTAs of a launch run in tile order and a tile's integral work grows with its points and with the pairs among the
+      // shells of B_j: heaviest tiles first inside every super-batch, so that the launch does not end on a few long CTAs.
+      for (const Super& sp : ctx->supers)
+        std::stable_sort(ctx->h_tiles.begin() + sp.t0, ctx->h_tiles.begin() + sp.t1, [&](const TileRec& x, const TileRec& y) {
+          return (double)x.n * h_bcnt[x.batch] * h_bcnt[x.batch] > (double)y.n * h_bcnt[y.batch] * h_bcnt[y.batch];
+        });
+      CK(upload(ctx->d_tiles, ctx->h_tiles));
       {   // a4 activity bits (density independent)
         std::vector<int64_t> h_bslot0(nb), h_btile0(nb);
         int64_t f = 0;

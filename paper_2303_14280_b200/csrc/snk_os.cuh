@@ -351,6 +351,9 @@ struct StoreSink {
 // halves the per-point cost of everything that does not depend on the point.
 // WARP: all 32 lanes call together; when every point of the warp is in the far field of a primitive pair (the common
 // case in the paper-shaped workloads) the Boys function runs without table loads or branches.
+#ifndef SNK_KP2_MAXL
+#define SNK_KP2_MAXL 1
+#endif
 #ifndef SNK_KP2_MAXNP
 #define SNK_KP2_MAXNP 1
 #endif
@@ -361,7 +364,7 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
   constexpr int L = LA + LB;
   // KP primitive pairs are advanced together: with the NP points that is KP*NP independent dependency chains per thread
   // (the FP64 pipe has an 8-cycle latency, a warp issues in order); the far-field vote is taken once for the group.
-  constexpr int KP = (WARP && L <= 1 && NP <= SNK_KP2_MAXNP) ? 2 : 1;
+  constexpr int KP = (WARP && L <= SNK_KP2_MAXL && NP <= SNK_KP2_MAXNP) ? 2 : 1;
 #pragma unroll
   for (int s = 0; s < NP; ++s)
 #pragma unroll
