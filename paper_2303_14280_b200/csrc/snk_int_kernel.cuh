@@ -3,7 +3,7 @@
 // up to kTile consecutive points of one batch.  A is never stored.
 //
 // B200 design (differs from the paper's A100 kernel):
-//   * warp-specialised: warps 0..CW-1 are consumers (CW = 8 for L <= 2, else 4), warp CW is a producer that walks the tile's V_j bit mask and streams
+//   * warp-specialised: warps 0..CW-1 are consumers (CW = 8, but 4 for L = 3 and L = 6), warp CW is a producer that walks the tile's V_j bit mask and streams
 //     every kept pair unit -- header + primitive pairs (<= 704 B) and the F_b rows of this tile -- into a ring of
 //     shared-memory slots with cp.async.bulk (TMA bulk copy) completing on an mbarrier; consumers never touch pair
 //     data in global memory, so the recurrences run against broadcast LDS only;
@@ -51,12 +51,15 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
 #ifndef SNK_MB_L2
 #define SNK_MB_L2 2
 #endif
+#ifndef SNK_MB_L4
+#define SNK_MB_L4 1
+#endif
 #ifndef SNK_MB_L3
 #define SNK_MB_L3 3
 #endif
 __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
   const int L = LA + LB;
-  return L == 0 ? SNK_MB_L0 : L == 1 ? SNK_MB_L1 : L == 2 ? SNK_MB_L2 : L == 3 ? SNK_MB_L3 : L == 4 ? 2 : 1;
+  return L == 0 ? SNK_MB_L0 : L == 1 ? SNK_MB_L1 : L == 2 ? SNK_MB_L2 : L == 3 ? SNK_MB_L3 : L == 4 ? SNK_MB_L4 : 1;
 }
 // consumer warps per CTA: NP per point group by default; more (SNK_CW_L*) let a group's unit stream be shared by more
 // warps, i.e. more resident point chains per staged unit and per producer warp
@@ -72,9 +75,18 @@ __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
 #ifndef SNK_CW_L3
 #define SNK_CW_L3 4
 #endif
+#ifndef SNK_CW_L4
+#define SNK_CW_L4 8
+#endif
+#ifndef SNK_CW_L5
+#define SNK_CW_L5 8
+#endif
+#ifndef SNK_CW_L6
+#define SNK_CW_L6 4
+#endif
 __host__ __device__ constexpr int int_cw(int LA, int LB) {
   const int L = LA + LB;
-  return L == 0 ? SNK_CW_L0 : L == 1 ? SNK_CW_L1 : L == 2 ? SNK_CW_L2 : L == 3 ? SNK_CW_L3 : 4;
+  return L == 0 ? SNK_CW_L0 : L == 1 ? SNK_CW_L1 : L == 2 ? SNK_CW_L2 : L == 3 ? SNK_CW_L3 : L == 4 ? SNK_CW_L4 : L == 5 ? SNK_CW_L5 : SNK_CW_L6;
 }
 __host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_cw(LA, LB) + 32; }
 
