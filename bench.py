@@ -296,6 +296,9 @@ def main():
                                          "flops": st["flops_integral"], "share_of_step": all_ms / st["ms_build"] if st["ms_build"] else None},
                 "gemm_dmma": {"peak": dmma_peak, "achieved": st["flops_gemm"] / ((st["ms_F"] + st["ms_Kt"] + 1e-12) * 1e-3) * 1e-12,
                               "ms_F": st["ms_F"], "ms_Kt": st["ms_Kt"]},
+                "per_class": {snk.CLASS_NAMES[c]: {"ms": st["ms_G_class"][c], "achieved": st["flops_class"][c] / (st["ms_G_class"][c] * 1e-3) * 1e-12,
+                                                   "frac": st["flops_class"][c] / (st["ms_G_class"][c] * 1e-3) * 1e-12 / dfma_peak if dfma_peak else None}
+                              for c in range(len(snk.CLASS_NAMES)) if st["ms_G_class"][c] > 0},
                 "flop_model": "far-field (asymptotic Boys) instruction count of the kernel templates, FMA = 2 (DESIGN.md)"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
