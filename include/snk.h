@@ -103,7 +103,9 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
 /* ---- snk_build_K: "Input: density matrix D ... Output: K" ---------------------
  *   P  DEVICE [nbf*nbf] row-major, symmetric (assumed, R7)    K  DEVICE [nbf*nbf], overwritten
  * Ordered on `stream`; K is valid when the stream reaches the end of the call's work.  The call reads back
- * a handful of list sizes (one small synchronisation) but never moves matrix data through the host. */
+ * a handful of list sizes (one small synchronisation) but never moves matrix data through the host.
+ * Environment: SNK_TRACE (any value) makes the call synchronise after every stage and report it on stderr
+ * (debugging aid; it perturbs the timings). */
 int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream);
 
 /* Same build with HOST buffers: H2D copy of P, build, D2H copy of K, stream synchronised on return.
