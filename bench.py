@@ -82,29 +82,34 @@ class ClockSampler:
 
 
 def time_oracle_sample(w, target_s=15.0, first_frac=0.01):
-    """Oracle (as it stands) on a bounded whole-root-cell sample sized for ~target_s of host time."""
+    """Oracle (as it stands) on a bounded sample sized for ~target_s of host time: whole root cells in R13 hash order; when even
+    the first cells are too much (config 4: 3.3e6 integrals per point) every k-th point of them."""
     from oracle import oracle as orc
     from paper_2303_14280_b200.dist import root_cell_sample
     o = orc.Oracle(w.basis)
+    npts = w.points.shape[0]
 
-    def run(frac):
-        m = root_cell_sample(w.points, w.batch_cell, frac) if frac < 1.0 else np.ones(w.points.shape[0], dtype=bool)
-        o.set_grid(w.points[m], w.weights[m], eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
+    def run(idx):
+        o.set_grid(w.points[idx], w.weights[idx], eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
         t = time.time()
         o.build_K(w.P)
-        dt = time.time() - t
-        st = o.stats()
-        return dt, st, int(m.sum())
+        return time.time() - t, o.stats()
 
-    dt, st, npt = run(first_frac)
-    rate = st["n_pairpoints"] / max(dt, 1e-6)
-    # second run sized from the first one's rate (pair-points per point assumed uniform)
-    frac = min(1.0, first_frac * target_s / max(dt, 1e-3))
-    if frac > 1.5 * first_frac:
-        dt, st, npt = run(frac)
+    idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, first_frac))[0] if first_frac < 1.0 else np.arange(npts)
+    probe = idx[::max(1, len(idx) // 128)]
+    dt0, _ = run(probe)
+    want = int(target_s * len(probe) / max(dt0, 1e-4))            # points the oracle can do in target_s
+    how = "whole root cells (R13 hash order)"
+    if want < len(idx):
+        idx = idx[::max(1, -(-len(idx) // max(want, 1)))]
+        how = "every k-th point of the first root cells (R13 hash order)"
+    elif want > 1.5 * len(idx) and first_frac < 1.0:
+        frac = min(1.0, first_frac * want / len(idx))
+        idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, frac))[0] if frac < 1.0 else np.arange(npts)
+    dt, st = run(idx)
     return dict(value=st["n_int_contracted"] / dt, unit=UNIT, cores=st["threads"], kind="oracle",
-                sample="whole root cells (R13 hash order): %d of %d points (%.2f%%), %.3g contracted integrals, %.2f s; "
-                       "oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % (npt, w.points.shape[0], 100.0 * npt / w.points.shape[0],
+                sample="%s: %d of %d points (%.3f%%), %.3g contracted integrals, %.2f s; "
+                       "oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % (how, len(idx), npts, 100.0 * len(idx) / npts,
                                                                                   st["n_int_contracted"], dt),
                 seconds=dt, n_int=st["n_int_contracted"])
 
