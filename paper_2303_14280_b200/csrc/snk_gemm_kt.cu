@@ -4,7 +4,8 @@
 //   * CTA tile 32 (Phi rows) x 256 (G rows), k-tile 16 slots, 8 warps (1 x 8), warp tile 32 x 32 = 4 x 4 fragments,
 //     accumulators in registers.  (64 x 256 with 2 x 4 warps has the better operand reuse but skips fewer blocks:
 //     490 vs 427 ms on cfg 3.)
-//   * Operand tiles travel global -> shared with 16-byte cp.async in a 4-stage ring (one __syncthreads per k-tile); the
+//   * Operand tiles travel global -> shared with 16-byte cp.async, double buffered (one __syncthreads per k-tile), two
+//     CTAs per SM (92 KB of shared memory and at most 128 registers each; a 4-stage ring with one CTA is 18 % slower); the
 //     shared rows keep the k-contiguous order with a row stride of 20 doubles, which makes the fragment loads
 //     (thread (g,t) reads [row g][k t]) hit 16 distinct 8-byte banks per half warp.
 //   * w_g is staged with the tile and folded into the Phi fragments.
@@ -64,9 +65,16 @@ struct BitWalk {
 #ifndef SNK_KT_TA
 #define SNK_KT_TA 32
 #endif
-constexpr int TA = SNK_KT_TA, TB = 256, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK, KT_STAGES = 4;
+constexpr int TA = SNK_KT_TA, TB = 256, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK;
+#ifndef SNK_KT_STAGES
+#define SNK_KT_STAGES 2
+#endif
+#ifndef SNK_KT_MINB
+#define SNK_KT_MINB 2
+#endif
+constexpr int KT_STAGES = SNK_KT_STAGES;
 constexpr int KT_WM = TA / 32, KT_WN = 8 / KT_WM, KT_NJ = TB / KT_WN / 8;   // warps along Phi rows / G rows, fragments per warp along G
-__global__ void __launch_bounds__(NTH) k_gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* __restrict__ Phi,
+__global__ void __launch_bounds__(NTH, SNK_KT_MINB) k_gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* __restrict__ Phi,
                                                  const double* __restrict__ G, int64_t ld, const double* __restrict__ wts,
                                                  double* __restrict__ Kt, const uint32_t* __restrict__ act, int64_t actw, int64_t wchunk) {
   extern __shared__ __align__(16) double smem_kt[];
