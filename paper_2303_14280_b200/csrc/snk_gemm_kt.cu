@@ -160,19 +160,30 @@ __global__ void __launch_bounds__(NTH, SNK_KT_MINB) k_gemm_kt(int64_t nbf, int64
   }
 }
 
-// a4:  F[lam, g] = sum_sigma P[lam, sigma] Phi[sigma, g]     Eq. 35/48.  Same pipeline; the B operand
+// a4:  F[lam, g] = sum_sigma P[lam, sigma] Phi[sigma, g]     Eq. 35/48.  CTA tile 64 x 128, double
+// buffered, three CTAs per SM; the B operand
 // (Phi rows) is contiguous along the output column g, so its shared tile is [16 k][132].  P has an arbitrary row stride
 // (nbf), hence 8-byte copies for it.  A bit per (128-slot column tile, 16-function k-tile) says whether Phi is non-zero
 // there (some shell overlapping the k-tile is in B_j of a batch overlapping the column tile); zero blocks are skipped.
 constexpr int LDN = 132;
-constexpr int FSTAGE_DOUBLES = TM * LDK + TK * LDN;
-__global__ void __launch_bounds__(NTH) k_gemm_f(int64_t nbf, int64_t ncols, const double* __restrict__ P, const double* __restrict__ Phi,
+#ifndef SNK_F_ROWS
+#define SNK_F_ROWS 64
+#endif
+#ifndef SNK_F_STAGES
+#define SNK_F_STAGES 2
+#endif
+#ifndef SNK_F_MINB
+#define SNK_F_MINB 3
+#endif
+constexpr int TMR = SNK_F_ROWS, FNI = TMR / 16, FST = SNK_F_STAGES;   // rows of the F tile, row fragments per warp, ring depth
+constexpr int FSTAGE_DOUBLES = TMR * LDK + TK * LDN;
+__global__ void __launch_bounds__(NTH, SNK_F_MINB) k_gemm_f(int64_t nbf, int64_t ncols, const double* __restrict__ P, const double* __restrict__ Phi,
                                                 double* __restrict__ F, int64_t ld, const uint32_t* __restrict__ act, int kwords) {
   extern __shared__ __align__(16) double smem_kt[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 2, wn = warp & 3;
   const int g = lane >> 2, t = lane & 3;
-  const int64_t n0 = (int64_t)blockIdx.x * TM, m0 = (int64_t)blockIdx.y * TM;
+  const int64_t n0 = (int64_t)blockIdx.x * TM, m0 = (int64_t)blockIdx.y * TMR;
   BitWalk walk;
   walk.init(act + (int64_t)blockIdx.x * kwords, 0, kwords, 0, (nbf + TK - 1) / TK);
   const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem_kt);
@@ -180,7 +191,7 @@ __global__ void __launch_bounds__(NTH) k_gemm_f(int64_t nbf, int64_t ncols, cons
     const int64_t k0 = kt * TK;
     const uint32_t sa = sbase + (uint32_t)(stage * FSTAGE_DOUBLES) * 8u;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {                          // A: 128 rows x 16 k, 8-byte copies
+    for (int i = 0; i < TMR * 16 / NTH; ++i) {             // A: TMR rows x 16 k, 8-byte copies
       const int c = tid + NTH * i, row = c >> 4, kc = c & 15;
       const int64_t r = m0 + row, k = k0 + kc;
       const bool ok = r < nbf && k < nbf;
@@ -193,46 +204,46 @@ __global__ void __launch_bounds__(NTH) k_gemm_f(int64_t nbf, int64_t ncols, cons
       const int c = tid + NTH * i, kr = c >> 6, nc = (c & 63) * 2;
       const int64_t k = k0 + kr, col = n0 + nc;
       const bool ok = k < nbf && col < ncols;
-      cp_async16(sa + (uint32_t)(TM * LDK + kr * LDN + nc) * 8u, Phi + (ok ? k * ld + col : 0), ok ? 16u : 0u);
+      cp_async16(sa + (uint32_t)(TMR * LDK + kr * LDN + nc) * 8u, Phi + (ok ? k * ld + col : 0), ok ? 16u : 0u);
     }
   };
-  double acc[8][4][2];
+  double acc[FNI][4][2];
 #pragma unroll
-  for (int i = 0; i < 8; ++i)
+  for (int i = 0; i < FNI; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
   int64_t pending = walk.next();
   int issued = 0;
 #pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) {
+  for (int s = 0; s < FST - 1; ++s) {
     if (pending >= 0) { issue(s, pending); ++issued; pending = walk.next(); }
     cp_commit();
   }
   for (int it = 0; it < issued; ++it) {
-    cp_wait<STAGES - 2>();
+    cp_wait<FST - 2>();
     __syncthreads();
-    if (pending >= 0) { issue((it + STAGES - 1) % STAGES, pending); ++issued; pending = walk.next(); }
+    if (pending >= 0) { issue((it + FST - 1) % FST, pending); ++issued; pending = walk.next(); }
     cp_commit();
-    const double* st = smem_kt + (it % STAGES) * FSTAGE_DOUBLES;
-    const double* as = st + (wm * 64 + g) * LDK + t;
-    const double* bs = st + TM * LDK + t * LDN + wn * 32 + g;
+    const double* st = smem_kt + (it % FST) * FSTAGE_DOUBLES;
+    const double* as = st + (wm * (TMR / 2) + g) * LDK + t;
+    const double* bs = st + TMR * LDK + t * LDN + wn * 32 + g;
 #pragma unroll
     for (int kk = 0; kk < TK; kk += 4) {
-      double af[8], bf[4];
+      double af[FNI], bf[4];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) af[i] = as[i * 8 * LDK + kk];
+      for (int i = 0; i < FNI; ++i) af[i] = as[i * 8 * LDK + kk];
 #pragma unroll
       for (int j = 0; j < 4; ++j) bf[j] = bs[kk * LDN + j * 8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i)
+      for (int i = 0; i < FNI; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     }
   }
   // F is overwritten (zeros where every block was skipped)
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int64_t row = m0 + wm * 64 + i * 8 + g;
+  for (int i = 0; i < FNI; ++i) {
+    const int64_t row = m0 + wm * (TMR / 2) + i * 8 + g;
     if (row >= nbf) continue;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -333,14 +344,14 @@ cudaError_t run_f_flags(const ShellTab& sh, int nbatch, const int32_t* bn, const
 cudaError_t gemm_f(int64_t nbf, int64_t ncols, const double* P, const double* Phi, double* F, int64_t ld, const uint32_t* act, int kwords,
                    cudaStream_t s) {
   if (nbf <= 0 || ncols <= 0) return cudaSuccess;
-  constexpr int smem = STAGES * FSTAGE_DOUBLES * (int)sizeof(double);
+  constexpr int smem = FST * FSTAGE_DOUBLES * (int)sizeof(double);
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(k_gemm_f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  dim3 grid((unsigned)((ncols + TM - 1) / TM), (unsigned)((nbf + TM - 1) / TM));
+  dim3 grid((unsigned)((ncols + TM - 1) / TM), (unsigned)((nbf + TMR - 1) / TMR));
   k_gemm_f<<<grid, NTH, smem, s>>>(nbf, ncols, P, Phi, F, ld, act, kwords);
   return cudaGetLastError();
 }
