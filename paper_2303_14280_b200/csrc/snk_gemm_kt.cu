@@ -1,11 +1,12 @@
 // snk_gemm_kt.cu -- a6:  Kt[mu,nu] += sum_g Phi[mu,g] w_g G[nu,g]        Eq. 39, fp64 DMMA (m8n8k4)
 //
 // Both operands are rows of the [nbf x ld] slabs of one super-batch, i.e. contiguous along the contraction index g.
-//   * CTA tile 32 (Phi rows) x 256 (G rows), k-tile 16 slots, 8 warps (1 x 8), warp tile 32 x 32 = 4 x 4 fragments,
+//   * CTA tile 32 (Phi rows) x 128 (G rows), k-tile 16 slots, 8 warps (1 x 8), warp tile 32 x 16 = 4 x 2 fragments,
 //     accumulators in registers.  (64 x 256 with 2 x 4 warps has the better operand reuse but skips fewer blocks:
 //     490 vs 427 ms on cfg 3.)
-//   * Operand tiles travel global -> shared with 16-byte cp.async, double buffered (one __syncthreads per k-tile), two
-//     CTAs per SM (92 KB of shared memory and at most 128 registers each; a 4-stage ring with one CTA is 18 % slower); the
+//   * Operand tiles travel global -> shared with 16-byte cp.async, double buffered (one __syncthreads per k-tile), four
+//     CTAs per SM (51 KB of shared memory each; 32 x 256 tiles with two CTAs are 8 % slower, a 4-stage ring with one
+//     CTA 25 %); the
 //     shared rows keep the k-contiguous order with a row stride of 20 doubles, which makes the fragment loads
 //     (thread (g,t) reads [row g][k t]) hit 16 distinct 8-byte banks per half warp.
 //   * w_g is staged with the tile and folded into the Phi fragments.
@@ -65,12 +66,15 @@ struct BitWalk {
 #ifndef SNK_KT_TA
 #define SNK_KT_TA 32
 #endif
-constexpr int TA = SNK_KT_TA, TB = 256, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK;
+#ifndef SNK_KT_TB
+#define SNK_KT_TB 128
+#endif
+constexpr int TA = SNK_KT_TA, TB = SNK_KT_TB, KT_STAGE_DOUBLES = (TA + TB) * LDK + TK;
 #ifndef SNK_KT_STAGES
 #define SNK_KT_STAGES 2
 #endif
 #ifndef SNK_KT_MINB
-#define SNK_KT_MINB 2
+#define SNK_KT_MINB 4
 #endif
 constexpr int KT_STAGES = SNK_KT_STAGES;
 constexpr int KT_WM = TA / 32, KT_WN = 8 / KT_WM, KT_NJ = TB / KT_WN / 8;   // warps along Phi rows / G rows, fragments per warp along G
