@@ -81,7 +81,7 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_oracle_sample(w, target_s=15.0, first_frac=0.01):
+def time_oracle_sample(w, target_s=15.0, first_frac=0.01, return_idx=False):
     """Oracle (as it stands) on a bounded sample sized for ~target_s of host time: whole root cells in R13 hash order; when even
     the first cells are too much (config 4: 3.3e6 integrals per point) every k-th point of them."""
     from oracle import oracle as orc
@@ -111,7 +111,8 @@ def time_oracle_sample(w, target_s=15.0, first_frac=0.01):
         frac = min(1.0, len(idx) / npts * target_s / max(dt, 1e-3))
         idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, frac))[0] if frac < 1.0 else np.arange(npts)
         dt, st = run(idx)
-    return dict(value=st["n_int_contracted"] / dt, unit=UNIT, cores=st["threads"], kind="oracle",
+    extra = {"idx": idx} if return_idx else {}
+    return dict(extra, value=st["n_int_contracted"] / dt, unit=UNIT, cores=st["threads"], kind="oracle",
                 sample="%s: %d of %d points (%.3f%%), %.3g contracted integrals, %.2f s; "
                        "oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % (how, len(idx), npts, 100.0 * len(idx) / npts,
                                                                                   st["n_int_contracted"], dt),
@@ -119,25 +120,36 @@ def time_oracle_sample(w, target_s=15.0, first_frac=0.01):
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle on the host cores, same config/metric; each step = a bounded sample."""
+    """--impl reference: the oracle on the host cores, same config/metric.  The sample is sized ONCE exactly as the
+    `cpu_baseline` leg of the GPU arm sizes it (whole root cells in R13 hash order, about --cpu-seconds of host time, no
+    thinning unless one root cell is already too much) and every step times the oracle's K build on that same sample, so the
+    rate is the cpu_baseline's rate; the grid is generated on the same device as in the GPU arm (same points and weights)."""
     if rank != 0:
         return
+    from oracle import oracle as orc
     from paper_2303_14280_b200 import inputs
-    w = inputs.make_workload(args.config, grid=args.grid, device="cpu" if args.config in (1, 2, 5) else _gen_device())
-    per_step = max(2.0, 120.0 / max(1, args.steps + args.warmup))
+    w = inputs.make_workload(args.config, grid=args.grid, device=_gen_device())
+    first = time_oracle_sample(w, target_s=args.cpu_seconds, return_idx=True)
+    idx = first.pop("idx")
+    o = orc.Oracle(w.basis)
+    o.set_grid(w.points[idx], w.weights[idx], eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
     res = []
     for i in range(args.warmup + args.steps):
-        r = time_oracle_sample(w, target_s=min(per_step, 20.0))
+        t = time.time()
+        o.build_K(w.P)
+        dt = time.time() - t
         if i >= args.warmup:
-            res.append(r)
-    n_int = sum(r["n_int"] for r in res)
-    secs = sum(r["seconds"] for r in res)
-    val = n_int / secs
+            res.append(dt)
+    st = o.stats()
+    n_int = st["n_int_contracted"]
+    secs = sum(res)
+    val = n_int * len(res) / secs
+    sample = first["sample"].split(", %.3g" % first["n_int"])[0] + ", %.3g contracted integrals per step; oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % n_int
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "strong",
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args.config, w), "sample": res[-1]["sample"]},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": res[-1]["cores"], "kind": "oracle", "sample": res[-1]["sample"]},
+            "config": {"workload": _workload_name(args.config, w), "sample": sample, "batch_cell": w.batch_cell, "batch_max": w.batch_max},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": st["threads"], "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
@@ -177,7 +189,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=3,
+                    help="BASELINE.json config 1..5; default 3 (64 waters, 1 600 functions, 3.9 M points): the largest configuration whose "
+                         "build (about 1.5 s) lets the driver's warm-up + timed steps and the e2e leg finish within minutes; config 4 "
+                         "(1 029 atoms) takes minutes per build and is run with --config 4 --steps 1")
     ap.add_argument("--grid", type=lambda s: tuple(int(x) for x in s.split(",")), default=None, help="override n_r,n_theta,n_phi")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -312,7 +327,11 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args.config, w), "l2": "working set (Phi, F, G slabs) far larger than the 126 MB L2; no flush needed",
+            "config": {"workload": _workload_name(args.config, w),
+                       "why_this_config": "largest single-GPU configuration of BASELINE.json whose K build (seconds) fits warm-up + timed steps + "
+                                          "the e2e leg in minutes; configs[3] (343 waters) costs minutes per build: `--config 4 --steps 1`, "
+                                          "summary under profiles/",
+                       "l2": "working set (Phi, F, G slabs) far larger than the 126 MB L2; no flush needed",
                        "parallelism": "1 GPU" if world == 1 else ("root cells -> %d ranks by Alg. 2 LPT, NCCL all-reduce of K per build" % world if shard else "%d independent replicas (own density each), no collective" % world),
                        "batch_cell": w.batch_cell, "batch_max": w.batch_max, "n_int_per_step": n_int, "n_int_primitive_per_step": n_prim,
                        "n_pairpoints_per_step": n_pp},

@@ -26,6 +26,7 @@ enum Stage { ST_SCREEN = 0, ST_COLLOC, ST_F, ST_G, ST_KT, ST_SYM, ST_COUNT };
 }  // namespace
 
 struct snk_ctx {
+  int device = -1;              // the CUDA device current at snk_create: every later call must run with it current
   int natoms = 0, nsh = 0, nbf = 0;
   std::vector<double> h_cx, h_cy, h_cz, h_pexp, h_pcoef;
   std::vector<int32_t> h_l, h_foff, h_poff, h_nprim;
@@ -86,9 +87,15 @@ struct snk_ctx {
     t.pexp = d_pexp.p; t.pcoef = d_pcoef.p; t.rcut2 = d_rcut2.p; t.nsh = nsh; t.nbf = nbf;
     return t;
   }
-  int new_event() {
-    if (ev_used == (int)ev_pool.size()) { cudaEvent_t e; cudaEventCreate(&e); ev_pool.push_back(e); }
-    return ev_used++;
+  cudaError_t new_event(int& id) {
+    if (ev_used == (int)ev_pool.size()) {
+      cudaEvent_t e;
+      const cudaError_t rc = cudaEventCreate(&e);
+      if (rc != cudaSuccess) return rc;
+      ev_pool.push_back(e);
+    }
+    id = ev_used++;
+    return cudaSuccess;
   }
 };
 
@@ -104,6 +111,14 @@ struct snk_ctx {
   } while (0)
 
 #define FAIL(code, msg) do { ctx->err = (msg); return (code); } while (0)
+
+// the context's buffers, events and shared-memory opt-ins belong to one device
+#define CHECK_DEVICE()                                                                                              \
+  do {                                                                                                              \
+    int d__ = -1;                                                                                                   \
+    if (cudaGetDevice(&d__) != cudaSuccess || d__ != ctx->device)                                                   \
+      FAIL(SNK_ESTATE, "the CUDA device that was current at snk_create must be current for every call on the context"); \
+  } while (0)
 
 namespace {
 
@@ -221,6 +236,25 @@ void class_flops(int la, int lb, double& per_prim, double& per_contr) {
 
 int set_err(snk_ctx* ctx, int code, const char* msg) { ctx->err = msg; return code; }
 
+// No exception crosses the C ABI (include/snk.h): host allocation failures become SNK_ENOMEM, anything else SNK_ECUDA
+// (std::system_error of a worker thread, ...) with the text in snk_last_error.
+template <class F>
+int guarded(snk_ctx* ctx, F&& body) {
+  auto note = [&](const char* what) { try { if (ctx) ctx->err = what; else g_create_error = what; } catch (...) {} };
+  try {
+    return body();
+  } catch (const std::bad_alloc&) {
+    note("out of host memory");
+    return SNK_ENOMEM;
+  } catch (const std::exception& e) {
+    note(e.what());
+    return SNK_ECUDA;
+  } catch (...) {
+    note("unknown C++ exception");
+    return SNK_ECUDA;
+  }
+}
+
 }  // namespace
 
 // ====================================================================================================================
@@ -251,14 +285,17 @@ void snk_destroy(snk_ctx* ctx) {
 
 int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t nshells, const int32_t* shell_atom,
                const int32_t* shell_l, const int32_t* shell_nprim, const double* prim_exp, const double* prim_coef) {
+  snk_ctx* ctx = nullptr;
+  const int rc = guarded(nullptr, [&]() -> int {
   if (out) *out = nullptr;
   if (!out || natoms < 1 || nshells < 1 || !atom_xyz || !shell_atom || !shell_l || !shell_nprim || !prim_exp || !prim_coef) {
     g_create_error = "snk_create: NULL argument or empty basis";
     return SNK_EINVAL;
   }
-  snk_ctx* ctx = new (std::nothrow) snk_ctx;
+  ctx = new (std::nothrow) snk_ctx;
   if (!ctx) { g_create_error = "snk_create: out of host memory"; return SNK_ENOMEM; }
-  auto bail = [&](int code, const std::string& m) { g_create_error = m; snk_destroy(ctx); return code; };
+  auto bail = [&](int code, const std::string& m) { g_create_error = m; snk_destroy(ctx); ctx = nullptr; return code; };
+  if (cudaGetDevice(&ctx->device) != cudaSuccess) return bail(SNK_ECUDA, "snk_create: no current CUDA device");
   ctx->natoms = natoms; ctx->nsh = nshells;
   int64_t po = 0;
   int fo = 0;
@@ -335,10 +372,15 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
     return bail(e == cudaErrorMemoryAllocation ? SNK_ENOMEM : SNK_ECUDA, std::string("snk_create: CUDA: ") + cudaGetErrorString(e));
   *out = ctx;
   return SNK_OK;
+  });
+  if (rc != SNK_OK && ctx) { snk_destroy(ctx); if (out) *out = nullptr; }    // an exception left a half-built context
+  return rc;
 }
 
 int snk_set_option(snk_ctx* ctx, const char* key, double value) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx || !key) return SNK_EINVAL;
+  CHECK_DEVICE();
   const std::string k(key);
   if (k == "eps") { if (!(value >= 0.0) || !std::isfinite(value)) FAIL(SNK_EINVAL, "eps must be finite and >= 0"); ctx->eps = value; }
   else if (k == "batch_cell") { if (!(value > 0.0) || !std::isfinite(value)) FAIL(SNK_EINVAL, "batch_cell must be > 0"); ctx->h0 = value; }
@@ -349,12 +391,15 @@ int snk_set_option(snk_ctx* ctx, const char* key, double value) {
   ctx->have_grid = false;      // options take effect at the next snk_set_grid
   ctx->have_build = false;
   return SNK_OK;
+  });
 }
 
 int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double* weights, void* stream_) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx) return SNK_EINVAL;
   if (npts < 0 || (npts > 0 && (!points || !weights))) FAIL(SNK_EINVAL, "snk_set_grid: bad npts / NULL pointer");
   if (npts >= ((int64_t)1 << 31) - 4096) FAIL(SNK_EINVAL, "snk_set_grid: more than 2^31 points");
+  CHECK_DEVICE();
   cudaStream_t s = (cudaStream_t)stream_;
   ctx->last_stream = s;
   ctx->have_grid = false; ctx->have_build = false; ctx->stats_valid = false;
@@ -554,11 +599,14 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
   ctx->stats.ms_set_grid = ms;
   ctx->have_grid = true;
   return SNK_OK;
+  });
 }
 
 int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx) return SNK_EINVAL;
   if (!P || !K) FAIL(SNK_EINVAL, "snk_build_K: NULL pointer");
+  CHECK_DEVICE();
   if (!ctx->have_grid) FAIL(SNK_ESTATE, "snk_build_K called before snk_set_grid");
   cudaStream_t s = (cudaStream_t)stream_;
   ctx->last_stream = s;
@@ -580,8 +628,20 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     const cudaError_t e = cudaStreamSynchronize(s);
     fprintf(stderr, "[snk] %s %d/%d: %s\n", what, a, b, cudaGetErrorString(e));
   };
-  auto span_begin = [&](int stage, int cls) { snk_ctx::Span sp{stage, cls, ctx->new_event(), -1}; cudaEventRecord(ctx->ev_pool[sp.e0], s); return sp; };
-  auto span_end = [&](snk_ctx::Span sp) { sp.e1 = ctx->new_event(); cudaEventRecord(ctx->ev_pool[sp.e1], s); ctx->spans.push_back(sp); };
+  cudaError_t span_rc = cudaSuccess;          // first failure of the timing events (checked with CK after every span)
+  auto span_begin = [&](int stage, int cls) {
+    snk_ctx::Span sp{stage, cls, -1, -1};
+    cudaError_t e = ctx->new_event(sp.e0);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_pool[sp.e0], s);
+    if (span_rc == cudaSuccess) span_rc = e;
+    return sp;
+  };
+  auto span_end = [&](snk_ctx::Span sp) {
+    cudaError_t e = ctx->new_event(sp.e1);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_pool[sp.e1], s);
+    if (span_rc == cudaSuccess) span_rc = e;
+    if (sp.e0 >= 0 && sp.e1 >= 0) ctx->spans.push_back(sp);
+  };
 
   // ---- a3: density-dependent screening (Eqs. 43-47) ----
   auto sp = span_begin(ST_SCREEN, -1);
@@ -670,14 +730,18 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   CK(run_symmetrise(nbf, ctx->d_Kt.p, K, s));
   ctx->n_launches += 1;
   span_end(sp);
+  CK(span_rc);
   CK(cudaEventRecord(ctx->ev_b1, s));
   ctx->have_build = true;
   return SNK_OK;
+  });
 }
 
 int snk_build_K_host(snk_ctx* ctx, const double* P_host, double* K_host, void* stream_) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx) return SNK_EINVAL;
   if (!P_host || !K_host) FAIL(SNK_EINVAL, "snk_build_K_host: NULL pointer");
+  CHECK_DEVICE();
   cudaStream_t s = (cudaStream_t)stream_;
   const size_t n = (size_t)ctx->nbf * ctx->nbf;
   CK(ctx->d_Pin.reserve(n)); CK(ctx->d_Kout.reserve(n));
@@ -687,10 +751,13 @@ int snk_build_K_host(snk_ctx* ctx, const double* P_host, double* K_host, void* s
   CK(cudaMemcpyAsync(K_host, ctx->d_Kout.p, n * sizeof(double), cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   return SNK_OK;
+  });
 }
 
 int snk_get_stats(snk_ctx* ctx, snk_stats* out) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx || !out) return SNK_EINVAL;
+  CHECK_DEVICE();
   cudaStream_t s = ctx->last_stream;
   CK(cudaStreamSynchronize(s));
   snk_stats& st = ctx->stats;
@@ -733,11 +800,14 @@ int snk_get_stats(snk_ctx* ctx, snk_stats* out) {
   }
   *out = st;
   return SNK_OK;
+  });
 }
 
 int snk_export_lists(snk_ctx* ctx, int64_t* sizes, int64_t* batch_off, int64_t* perm, int64_t* B_off, int32_t* B_ids, int64_t* V_off,
                      int32_t* V_pairs) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx || !sizes) return SNK_EINVAL;
+  CHECK_DEVICE();
   if (!ctx->have_grid) FAIL(SNK_ESTATE, "snk_export_lists before snk_set_grid");
   cudaStream_t s = ctx->last_stream;
   CK(cudaStreamSynchronize(s));
@@ -790,20 +860,28 @@ int snk_export_lists(snk_ctx* ctx, int64_t* sizes, int64_t* batch_off, int64_t* 
     if (V_off) V_off[nb] = o;
   } else if (V_off) V_off[0] = 0;
   return SNK_OK;
+  });
 }
 
 int snk_debug_boys(int32_t mmax, int64_t n, const double* x, double* out, void* stream_) {
+  return guarded((snk_ctx*)nullptr, [&]() -> int {
   if (mmax < 0 || mmax > 6 || n < 0 || (n > 0 && (!x || !out))) return SNK_EINVAL;
-  static DevBuf<double> tab;      // process-lifetime table for the hook
+  static DevBuf<double> tabs[kMaxDevices];      // process-lifetime table of the hook, one per device
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return SNK_ECUDA;
+  DevBuf<double>& tab = tabs[dev];
   if (!tab.p) {
     if (upload(tab, make_boys_table()) != cudaSuccess) return SNK_ECUDA;
   }
   return launch_debug_boys(mmax, n, x, tab.p, out, (cudaStream_t)stream_) == cudaSuccess ? SNK_OK : SNK_ECUDA;
+  });
 }
 
 int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double* pts, double* out, void* stream_) {
+  return guarded(ctx, [&]() -> int {
   if (!ctx) return SNK_EINVAL;
   if (a < 0 || b < 0 || a >= ctx->nsh || b >= ctx->nsh || n < 0 || (n > 0 && (!pts || !out))) FAIL(SNK_EINVAL, "snk_debug_A_pair: bad argument");
+  CHECK_DEVICE();
   cudaStream_t s = (cudaStream_t)stream_;
   const bool tr = ctx->h_l[a] < ctx->h_l[b];
   const int sa = tr ? b : a, sb = tr ? a : b;
@@ -830,11 +908,14 @@ int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double
   d.release();
   CK(e); CK(e2);
   return SNK_OK;
+  });
 }
 
 int snk_measure_fp64_peak(double* dfma_tflops, double* dmma_tflops, int32_t reps) {
+  return guarded((snk_ctx*)nullptr, [&]() -> int {
   if (!dfma_tflops || !dmma_tflops || reps < 1) return SNK_EINVAL;
   return run_fp64_peak(dfma_tflops, dmma_tflops, reps) == cudaSuccess ? SNK_OK : SNK_ECUDA;
+  });
 }
 
 }  // extern "C"

@@ -151,8 +151,8 @@ cudaError_t gemm_f64(bool transB, int64_t M, int64_t N, int64_t K, const double*
   // split-K when the output is too small to fill the GPU (the Kt contraction: M = N = nbf, K = grid points)
   int64_t kchunk = K > 0 ? K : 1;
   if (beta && K > 0) {
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    int sms = 0, dev = 0;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int64_t ctas = (int64_t)grid.x * grid.y;
     int64_t split = (2 * sms + ctas - 1) / ctas;
     split = std::max<int64_t>(1, std::min<int64_t>(split, K / (8 * BK)));
@@ -160,12 +160,9 @@ cudaError_t gemm_f64(bool transB, int64_t M, int64_t N, int64_t K, const double*
     grid.z = (unsigned)((K + kchunk - 1) / kchunk);
   }
   constexpr int smem = 4 * BK * LDS * (int)sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_gemm_f64<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(k_gemm_f64<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    attr_set = true;
-  }
+  static bool attr_t[kMaxDevices] = {}, attr_n[kMaxDevices] = {};
+  if (cudaError_t e = opt_in_smem(k_gemm_f64<true>, smem, attr_t); e != cudaSuccess) return e;
+  if (cudaError_t e = opt_in_smem(k_gemm_f64<false>, smem, attr_n); e != cudaSuccess) return e;
   if (transB) k_gemm_f64<true><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale, kchunk);
   else k_gemm_f64<false><<<grid, NT, smem, s>>>(M, N, K, A, lda, B, ldb, C, ldc, beta, kscale, kchunk);
   return cudaGetLastError();

@@ -326,12 +326,8 @@ cudaError_t gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* Ph
   while (wchunk > 2 && 2.0 * nbf * (double)wchunk * 512 * 8 > 48e6) wchunk /= 2;
   const int64_t split = (nwords + wchunk - 1) / wchunk;
   constexpr int smem = KT_STAGES * KT_STAGE_DOUBLES * (int)sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_gemm_kt, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static bool attr_set[kMaxDevices] = {};
+  if (cudaError_t e = opt_in_smem(k_gemm_kt, smem, attr_set); e != cudaSuccess) return e;
   dim3 grid((unsigned)ntb, (unsigned)nta, (unsigned)split);
   k_gemm_kt<<<grid, NTH, smem, s>>>(nbf, slot0, nslots, Phi, G, ld, wts, Kt, act, actw, wchunk);
   return cudaGetLastError();
@@ -349,12 +345,8 @@ cudaError_t gemm_f(int64_t nbf, int64_t ncols, const double* P, const double* Ph
                    cudaStream_t s) {
   if (nbf <= 0 || ncols <= 0) return cudaSuccess;
   constexpr int smem = FST * FSTAGE_DOUBLES * (int)sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_gemm_f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  static bool attr_set[kMaxDevices] = {};
+  if (cudaError_t e = opt_in_smem(k_gemm_f, smem, attr_set); e != cudaSuccess) return e;
   dim3 grid((unsigned)((ncols + TM - 1) / TM), (unsigned)((nbf + TMR - 1) / TMR));
   k_gemm_f<<<grid, NTH, smem, s>>>(nbf, ncols, P, Phi, F, ld, act, kwords);
   return cudaGetLastError();

@@ -372,12 +372,8 @@ template <int LA, int LB>
 cudaError_t launch_class(const IntParams& p, cudaStream_t s) {
   if (p.ntiles > 0 && p.pend > p.pbeg) {
     constexpr int smem = int_smem_bytes(LA, LB);
-    static bool attr_set = false;
-    if (!attr_set) {
-      cudaError_t e = cudaFuncSetAttribute(k_integrals<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-      if (e != cudaSuccess) return e;
-      attr_set = true;
-    }
+    static bool attr_set[kMaxDevices] = {};
+    if (cudaError_t e = opt_in_smem(k_integrals<LA, LB>, smem, attr_set); e != cudaSuccess) return e;
     k_integrals<LA, LB><<<p.ntiles, int_threads(LA, LB), smem, s>>>(p);
   }
   return cudaGetLastError();

@@ -76,6 +76,20 @@ struct DevBuf {           // grow-only device buffer
   ~DevBuf() { release(); }
 };
 
+// cudaFuncSetAttribute is per device: one opt-in flag per (kernel, device).  `done` is the call site's static table.
+constexpr int kMaxDevices = 64;
+template <class Kern>
+inline cudaError_t opt_in_smem(Kern kern, int bytes, bool (&done)[kMaxDevices]) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool tracked = dev >= 0 && dev < kMaxDevices;
+  if (tracked && done[dev]) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess && tracked) done[dev] = true;
+  return e;
+}
+
 struct IntParams {
   const double* gx; const double* gy; const double* gz;
   const double* F; double* G;
