@@ -59,6 +59,7 @@ def _load():
     lib.orc_screen.argtypes = [C.c_void_p, dp]
     lib.orc_build_K.argtypes = [C.c_void_p, dp, dp, C.c_int, ip]
     lib.orc_get_stats.argtypes = [C.c_void_p, dp]
+    lib.orc_set_extended.argtypes = [C.c_void_p, C.c_int]
     _lib = lib
     return lib
 
@@ -144,8 +145,11 @@ class Oracle:
         self._grid = True
         self.npts = pts.shape[0]
 
-    def build_K(self, P, sel_shells=None) -> np.ndarray:
+    def build_K(self, P, sel_shells=None, extended=False) -> np.ndarray:
+        """Eqs. 31-40.  ``extended``: the sums over sigma, lambda and g in long double (same terms, same order): a
+        rounding-order check of the fp64 result, not a different method."""
         assert self._grid
+        _lib.orc_set_extended(self.h, 1 if extended else 0)
         P = np.ascontiguousarray(P, dtype=np.float64)
         assert P.shape == (self.nbf, self.nbf)
         K = np.zeros((self.nbf, self.nbf))

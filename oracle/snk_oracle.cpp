@@ -275,6 +275,7 @@ struct Ctx {
   int nmax = 2048;
   std::vector<Batch> batches;
   std::vector<double> Abound;        // [nsh*nsh]
+  bool extended = false;             // orc_set_extended
   // stats of the last build
   double n_int_contr = 0, n_int_prim = 0, n_pairpoints = 0;
   double t_build = 0;
@@ -405,6 +406,105 @@ void do_pair_screen(Ctx& c, const double* P) {
 // =====================================================================================
 // C entry points (ctypes).  All arrays host, row-major, double / int32 / int64 as named.
 // =====================================================================================
+// The batch loop of orc_build_K (Eqs. 31, 35/48, 37-39), with the accumulator type R of the three sums over sigma, lambda and
+// g as a parameter.  R = double is the oracle proper.  R = long double evaluates the SAME terms in the SAME order with 64-bit
+// mantissas: it changes rounding only and exists to tell which side owns a difference of the size of the fp64 summation error
+// (DESIGN.md section 6); the A integrals and Phi stay fp64 in both.
+template <class R>
+static void build_batches(Ctx* c, const double* P, const std::vector<char>& insel, std::vector<std::vector<long double>>& Kacc,
+                          std::vector<double>& st_contr, std::vector<double>& st_prim, std::vector<double>& st_pp) {
+  const int nbf = c->nbf;
+  const int64_t nb = (int64_t)c->batches.size();
+#pragma omp parallel
+  {
+    int tid = 0;
+#ifdef _OPENMP
+    tid = omp_get_thread_num();
+#endif
+    std::vector<long double>& Kt = Kacc[tid];
+    Kt.assign((size_t)nbf * nbf, 0.0L);
+    std::vector<double> Phi, Ablk(100), val(10);
+    std::vector<R> F, G, Kj;
+    std::vector<PrimPair> pps;
+#pragma omp for schedule(dynamic)
+    for (int64_t j = 0; j < nb; ++j) {
+      const Batch& b = c->batches[j];
+      const int64_t nq = (int64_t)b.pts.size();
+      // packed function list of B_j
+      std::vector<int> bf;
+      for (int a : b.B) for (int i = 0; i < ncart(c->sh[a].l); ++i) bf.push_back(c->sh[a].foff + i);
+      const int nB = (int)bf.size();
+      // Eq. 31 / 42: Phi^(j)[g, k], k over functions of B_j
+      Phi.assign((size_t)nq * nB, 0.0);
+      for (int64_t g = 0; g < nq; ++g) {
+        int k = 0;
+        for (int a : b.B) {
+          shell_values(c->sh[a], &c->pts[3 * b.pts[g]], val.data());
+          for (int i = 0; i < ncart(c->sh[a].l); ++i) Phi[(size_t)g * nB + k++] = val[i];
+        }
+      }
+      // which functions lambda appear in V_j (as a partner we need F for)
+      std::vector<char> needF(nbf, 0);
+      for (auto& ab : b.V) {
+        if (!(insel[ab[0]] || insel[ab[1]])) continue;
+        for (int s2 = 0; s2 < 2; ++s2) for (int i = 0; i < ncart(c->sh[ab[s2]].l); ++i) needF[c->sh[ab[s2]].foff + i] = 1;
+      }
+      // Eq. 35 / 48: F[g, lam] = sum_{sigma in B_j} P[lam, sigma] Phi[g, sigma]
+      F.assign((size_t)nq * nbf, R(0));
+      for (int64_t g = 0; g < nq; ++g)
+        for (int lam = 0; lam < nbf; ++lam) {
+          if (!needF[lam]) continue;
+          R s = 0;
+          for (int k = 0; k < nB; ++k) s += (R)P[(size_t)lam * nbf + bf[k]] * (R)Phi[(size_t)g * nB + k];
+          F[(size_t)g * nbf + lam] = s;
+        }
+      // Eq. 37 + 38: G[g, nu] = w_g sum_lam A[g, nu, lam] F[g, lam] over pairs in V_j (both directions, R8)
+      G.assign((size_t)nq * nbf, R(0));
+      for (auto& ab : b.V) {
+        const int a = ab[0], bb = ab[1];
+        if (!(insel[a] || insel[bb])) continue;
+        const Shell& sa = c->sh[a]; const Shell& sb = c->sh[bb];
+        const int na = ncart(sa.l), nbc = ncart(sb.l);
+        make_prim_pairs(sa, sb, pps);
+        st_contr[tid] += (double)nq * na * nbc;
+        st_prim[tid] += (double)nq * na * nbc * sa.nprim * sb.nprim;
+        st_pp[tid] += (double)nq;
+        for (int64_t g = 0; g < nq; ++g) {
+          const int64_t gi = b.pts[g];
+          A_block(pps, na, nbc, &c->pts[3 * gi], Ablk.data());
+          const double wg = c->w[gi];
+          R* Gg = &G[(size_t)g * nbf];
+          const R* Fg = &F[(size_t)g * nbf];
+          if (insel[a])
+            for (int i = 0; i < na; ++i) {
+              R s = 0;
+              for (int k = 0; k < nbc; ++k) s += (R)Ablk[i * nbc + k] * Fg[sb.foff + k];
+              Gg[sa.foff + i] += (R)wg * s;
+            }
+          if (a != bb && insel[bb])
+            for (int k = 0; k < nbc; ++k) {
+              R s = 0;
+              for (int i = 0; i < na; ++i) s += (R)Ablk[i * nbc + k] * Fg[sa.foff + i];
+              Gg[sb.foff + k] += (R)wg * s;
+            }
+        }
+      }
+      // Eq. 39: Kt[mu, nu] += sum_g Phi[g, mu] G[g, nu],  mu in B_j
+      Kj.assign((size_t)nB * nbf, R(0));
+      for (int64_t g = 0; g < nq; ++g)
+        for (int k = 0; k < nB; ++k) {
+          const double ph = Phi[(size_t)g * nB + k];
+          if (ph == 0.0) continue;
+          R* row = &Kj[(size_t)k * nbf];
+          const R* Gg = &G[(size_t)g * nbf];
+          for (int nu = 0; nu < nbf; ++nu) row[nu] += (R)ph * Gg[nu];
+        }
+      for (int k = 0; k < nB; ++k)
+        for (int nu = 0; nu < nbf; ++nu) Kt[(size_t)bf[k] * nbf + nu] += (long double)Kj[(size_t)k * nbf + nu];
+    }
+  }
+}
+
 extern "C" {
 
 int orc_boys(int mmax, double x, double* F) {
@@ -550,93 +650,8 @@ int orc_build_K(void* h, const double* P, double* K, int nsel, const int32_t* se
 #ifdef _OPENMP
   const double t0 = omp_get_wtime();
 #endif
-#pragma omp parallel
-  {
-    int tid = 0;
-#ifdef _OPENMP
-    tid = omp_get_thread_num();
-#endif
-    std::vector<long double>& Kt = Kacc[tid];
-    Kt.assign((size_t)nbf * nbf, 0.0L);
-    std::vector<double> Phi, F, G, Kj, Ablk(100), val(10);
-    std::vector<PrimPair> pps;
-#pragma omp for schedule(dynamic)
-    for (int64_t j = 0; j < nb; ++j) {
-      const Batch& b = c->batches[j];
-      const int64_t nq = (int64_t)b.pts.size();
-      // packed function list of B_j
-      std::vector<int> bf;
-      for (int a : b.B) for (int i = 0; i < ncart(c->sh[a].l); ++i) bf.push_back(c->sh[a].foff + i);
-      const int nB = (int)bf.size();
-      // Eq. 31 / 42: Phi^(j)[g, k], k over functions of B_j
-      Phi.assign((size_t)nq * nB, 0.0);
-      for (int64_t g = 0; g < nq; ++g) {
-        int k = 0;
-        for (int a : b.B) {
-          shell_values(c->sh[a], &c->pts[3 * b.pts[g]], val.data());
-          for (int i = 0; i < ncart(c->sh[a].l); ++i) Phi[(size_t)g * nB + k++] = val[i];
-        }
-      }
-      // which functions lambda appear in V_j (as a partner we need F for)
-      std::vector<char> needF(nbf, 0);
-      for (auto& ab : b.V) {
-        if (!(insel[ab[0]] || insel[ab[1]])) continue;
-        for (int s2 = 0; s2 < 2; ++s2) for (int i = 0; i < ncart(c->sh[ab[s2]].l); ++i) needF[c->sh[ab[s2]].foff + i] = 1;
-      }
-      // Eq. 35 / 48: F[g, lam] = sum_{sigma in B_j} P[lam, sigma] Phi[g, sigma]
-      F.assign((size_t)nq * nbf, 0.0);
-      for (int64_t g = 0; g < nq; ++g)
-        for (int lam = 0; lam < nbf; ++lam) {
-          if (!needF[lam]) continue;
-          double s = 0.0;
-          for (int k = 0; k < nB; ++k) s += P[(size_t)lam * nbf + bf[k]] * Phi[(size_t)g * nB + k];
-          F[(size_t)g * nbf + lam] = s;
-        }
-      // Eq. 37 + 38: G[g, nu] = w_g sum_lam A[g, nu, lam] F[g, lam] over pairs in V_j (both directions, R8)
-      G.assign((size_t)nq * nbf, 0.0);
-      for (auto& ab : b.V) {
-        const int a = ab[0], bb = ab[1];
-        if (!(insel[a] || insel[bb])) continue;
-        const Shell& sa = c->sh[a]; const Shell& sb = c->sh[bb];
-        const int na = ncart(sa.l), nbc = ncart(sb.l);
-        make_prim_pairs(sa, sb, pps);
-        st_contr[tid] += (double)nq * na * nbc;
-        st_prim[tid] += (double)nq * na * nbc * sa.nprim * sb.nprim;
-        st_pp[tid] += (double)nq;
-        for (int64_t g = 0; g < nq; ++g) {
-          const int64_t gi = b.pts[g];
-          A_block(pps, na, nbc, &c->pts[3 * gi], Ablk.data());
-          const double wg = c->w[gi];
-          double* Gg = &G[(size_t)g * nbf];
-          const double* Fg = &F[(size_t)g * nbf];
-          if (insel[a])
-            for (int i = 0; i < na; ++i) {
-              double s = 0.0;
-              for (int k = 0; k < nbc; ++k) s += Ablk[i * nbc + k] * Fg[sb.foff + k];
-              Gg[sa.foff + i] += wg * s;
-            }
-          if (a != bb && insel[bb])
-            for (int k = 0; k < nbc; ++k) {
-              double s = 0.0;
-              for (int i = 0; i < na; ++i) s += Ablk[i * nbc + k] * Fg[sa.foff + i];
-              Gg[sb.foff + k] += wg * s;
-            }
-        }
-      }
-      // Eq. 39: Kt[mu, nu] += sum_g Phi[g, mu] G[g, nu],  mu in B_j
-      Kj.assign((size_t)nB * nbf, 0.0);
-      for (int64_t g = 0; g < nq; ++g)
-        for (int k = 0; k < nB; ++k) {
-          const double ph = Phi[(size_t)g * nB + k];
-          if (ph == 0.0) continue;
-          double* row = &Kj[(size_t)k * nbf];
-          const double* Gg = &G[(size_t)g * nbf];
-          for (int nu = 0; nu < nbf; ++nu) row[nu] += ph * Gg[nu];
-        }
-      for (int k = 0; k < nB; ++k)
-        for (int nu = 0; nu < nbf; ++nu) Kt[(size_t)bf[k] * nbf + nu] += (long double)Kj[(size_t)k * nbf + nu];
-    }
-  }
+  if (c->extended) build_batches<long double>(c, P, insel, Kacc, st_contr, st_prim, st_pp);
+  else build_batches<double>(c, P, insel, Kacc, st_contr, st_prim, st_pp);
   // reduce the per-thread accumulators in fixed thread order
   std::vector<long double> Kt((size_t)nbf * nbf, 0.0L);
   for (int t = 0; t < nthreads; ++t)
@@ -655,6 +670,9 @@ int orc_build_K(void* h, const double* P, double* K, int nsel, const int32_t* se
 #endif
   return 0;
 }
+
+// 1: the sums over sigma, lambda and g of the next orc_build_K run in long double (rounding-order check only); 0: fp64 (default)
+int orc_set_extended(void* h, int flag) { ((Ctx*)h)->extended = flag != 0; return 0; }
 
 // stats of the last orc_build_K: contracted integrals, primitive integrals, pair-points, seconds, threads
 int orc_get_stats(void* h, double* out5) {

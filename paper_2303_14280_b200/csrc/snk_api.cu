@@ -63,6 +63,7 @@ struct snk_ctx {
   DevBuf<unsigned char> d_units;                    // [nunit][kUnitBytes]
   DevBuf<UnitMeta> d_meta;                          // [nunit]
   DevBuf<uint32_t> d_vmask;
+  DevBuf<int32_t> d_vlist, d_vcnt;                  // unit-id lists of the current super-batch (k_vlist)
   DevBuf<char> d_tmp;
   int64_t vstride = 0;
   int npair_sig = 0, nunit = 0;
@@ -277,7 +278,7 @@ void snk_destroy(snk_ctx* ctx) {
   ctx->d_absP.release(); ctx->d_Ftf.release(); ctx->d_FtsT.release(); ctx->d_Kt.release();
   ctx->d_Pin.release(); ctx->d_Kout.release(); ctx->d_stats.release(); ctx->d_cflops.release();
   ctx->d_flag.release(); ctx->d_np.release(); ctx->d_pos.release(); ctx->d_ppos.release(); ctx->d_units.release();
-  ctx->d_meta.release(); ctx->d_vmask.release(); ctx->d_tmp.release();
+  ctx->d_meta.release(); ctx->d_vmask.release(); ctx->d_vlist.release(); ctx->d_vcnt.release(); ctx->d_tmp.release();
   for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
   for (cudaEvent_t e : {ctx->ev_b0, ctx->ev_b1, ctx->ev_g0, ctx->ev_g1}) if (e) cudaEventDestroy(e);
   delete ctx;
@@ -678,6 +679,11 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   ctx->vstride = (nunit + 31) / 32 + 1;
   CK(ctx->d_units.reserve((size_t)std::max(nunit, 1) * kUnitBytes)); CK(ctx->d_meta.reserve(std::max(nunit, 1)));
   CK(ctx->d_vmask.reserve((size_t)nb * ctx->vstride));
+  {   // unit-id lists: one row of nunit ints per batch of the largest super-batch (a class's slot is as long as the class)
+    int max_nb = 1;
+    for (const Super& su : ctx->supers) max_nb = std::max(max_nb, su.b1 - su.b0);
+    CK(ctx->d_vlist.reserve((size_t)max_nb * std::max(nunit, 1))); CK(ctx->d_vcnt.reserve((size_t)max_nb * kNumClasses));
+  }
   CK(run_unit_fill(ctx->cand, tab, ctx->d_flag.p, ctx->d_pos.p, ctx->d_Atil.p, 1e-4 * ctx->eps, (const double*)ctx->d_Fmax.p,
                    (const double*)ctx->d_phimax.p, ctx->ld, ctx->d_units.p, ctx->d_meta.p, s));
   CK(cudaMemsetAsync(ctx->d_vmask.p, 0, (size_t)nb * ctx->vstride * sizeof(uint32_t), s));
@@ -705,10 +711,13 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     CK(cudaMemsetAsync(ctx->d_G.p, 0, (size_t)nbf * ctx->ld * sizeof(double), s));
     IntParams ip;
     ip.gx = ctx->gx.p; ip.gy = ctx->gy.p; ip.gz = ctx->gz.p; ip.F = ctx->d_F.p; ip.G = ctx->d_G.p; ip.ld = ctx->ld; ip.slot0 = su.slot0;
-    ip.tiles = ctx->d_tiles.p + su.t0; ip.ntiles = ntiles; ip.vmask = ctx->d_vmask.p; ip.vstride = ctx->vstride;
+    ip.tiles = ctx->d_tiles.p + su.t0; ip.ntiles = ntiles;
+    CK(run_vlist(su.b0, su.b1 - su.b0, ctx->cls_beg, ctx->d_vmask.p, ctx->vstride, ctx->d_vlist.p, nunit, ctx->d_vcnt.p, s));
+    ctx->n_launches += 1;
+    ip.vlist = ctx->d_vlist.p; ip.vlstride = nunit; ip.vcnt = ctx->d_vcnt.p; ip.b0 = su.b0;
     ip.units = ctx->d_units.p; ip.meta = ctx->d_meta.p; ip.boys = ctx->d_boys.p;
     for (int c = 0; c < kNumClasses; ++c) {
-      ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1];
+      ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1]; ip.cls = c;
       if (ip.pend <= ip.pbeg) continue;
       auto spc = span_begin(ST_COUNT, c);
       CK(launch_integrals(c, ip, s));

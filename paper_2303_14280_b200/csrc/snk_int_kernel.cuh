@@ -1,15 +1,17 @@
 // snk_int_kernel.cuh -- integral-contraction kernel (row a5):  G[nu][g] += sum_{(nu,lam) in V_j} A_{nu,lam}(g) F[lam][g]
-// Eq. 38/48 via App. A.  One consumer thread = one grid point, one CTA = one tile of
+// Eq. 38/48 via App. A.  One consumer thread = NP grid points (PAPER.md:490 has one), one CTA = one tile of
 // up to kTile consecutive points of one batch.  A is never stored.
 //
 // B200 design (differs from the paper's A100 kernel):
-//   * warp-specialised: warps 0..CW-1 are consumers (CW = 8, but 4 for L = 3 and L = 6), warp CW is a producer that walks the tile's V_j bit mask and streams
-//     every kept pair unit -- header + primitive pairs (<= 704 B) and the F_b rows of this tile -- into a ring of
-//     shared-memory slots with cp.async.bulk (TMA bulk copy) completing on an mbarrier; consumers never touch pair
-//     data in global memory, so the recurrences run against broadcast LDS only;
-//   * a consumer thread owns NP points of the tile (2 for L <= 1, else 1) and the warps that cover the same points
-//     (4 of the 8 consumer warps for L <= 1, 2 for L = 2) split the unit stream dynamically (shared-memory ticket): the
-//     point-independent work of a unit is paid once per 32 NP points and one staged unit feeds more resident chains;
+//   * the V_j bit masks are expanded once per super-batch into per-(batch, class) unit-id lists (k_vlist); the warps of a tile
+//     that cover the same points (a point group: 4 of the 8 warps for L <= 1, 2 for L = 2) take the list's entries round robin;
+//   * every warp streams ITS units -- header + primitive pairs (<= 704 B) and the F_b row segments of its points -- through a
+//     private ring of D shared-memory slots with cp.async.bulk (TMA bulk copy) completing on a per-slot mbarrier: lane 0 refills
+//     a slot as soon as the warp has finished the unit in it, D units ahead, so the recurrences run against broadcast LDS only
+//     and never wait for global memory.  No producer warp (a ninth warp costs every thread of the CTA a quarter of its registers:
+//     CTAs are allocated in warp pairs), no tickets, no barrier shared between warps;
+//   * a thread owns NP points of the tile (2 for L <= 1, else 1): the point-independent work of a unit is paid once per 32 NP
+//     points and the NP recurrences are independent instruction streams;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
 //     fire-and-forget RED.F64 (coalesced along the slot index);
 //   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh).
@@ -26,13 +28,13 @@ namespace snk {
 // NP recurrences are independent instruction streams.  The tile is therefore covered by G = 4 / NP point groups of NP warps
 // each, and the warps of one group share the unit stream: each takes the next unit nobody of its group has taken yet.
 #ifndef SNK_NP_L0
-#define SNK_NP_L0 2
+#define SNK_NP_L0 4
 #endif
 #ifndef SNK_NP_L1
-#define SNK_NP_L1 2
+#define SNK_NP_L1 4
 #endif
 #ifndef SNK_NP_L2
-#define SNK_NP_L2 1
+#define SNK_NP_L2 2
 #endif
 #ifndef SNK_NP_L3
 #define SNK_NP_L3 1
@@ -41,36 +43,36 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
   const int L = LA + LB;
   return L == 0 ? SNK_NP_L0 : L == 1 ? SNK_NP_L1 : L == 2 ? SNK_NP_L2 : L == 3 ? SNK_NP_L3 : 1;
 }
-// resident CTAs per SM the register allocation is held to
+// resident CTAs per SM the register allocation is held to (8 warps per CTA: 2 CTAs = 4 warps per sub-partition = 128 registers)
 #ifndef SNK_MB_L0
-#define SNK_MB_L0 3
+#define SNK_MB_L0 2
 #endif
 #ifndef SNK_MB_L1
-#define SNK_MB_L1 2
+#define SNK_MB_L1 3
 #endif
 #ifndef SNK_MB_L2
-#define SNK_MB_L2 2
-#endif
-#ifndef SNK_MB_L4
-#define SNK_MB_L4 1
+#define SNK_MB_L2 3
 #endif
 #ifndef SNK_MB_L3
 #define SNK_MB_L3 3
+#endif
+#ifndef SNK_MB_L4
+#define SNK_MB_L4 1
 #endif
 __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
   const int L = LA + LB;
   return L == 0 ? SNK_MB_L0 : L == 1 ? SNK_MB_L1 : L == 2 ? SNK_MB_L2 : L == 3 ? SNK_MB_L3 : L == 4 ? SNK_MB_L4 : 1;
 }
-// consumer warps per CTA: NP per point group by default; more (SNK_CW_L*) let a group's unit stream be shared by more
-// warps, i.e. more resident point chains per staged unit and per producer warp
+// warps per CTA (all of them consume): NP per point group at least; more (SNK_CW_L*) let a group's unit stream be shared by
+// more warps, i.e. more resident point chains per staged unit
 #ifndef SNK_CW_L0
 #define SNK_CW_L0 8
 #endif
 #ifndef SNK_CW_L1
-#define SNK_CW_L1 8
+#define SNK_CW_L1 4
 #endif
 #ifndef SNK_CW_L2
-#define SNK_CW_L2 8
+#define SNK_CW_L2 4
 #endif
 #ifndef SNK_CW_L3
 #define SNK_CW_L3 4
@@ -88,18 +90,28 @@ __host__ __device__ constexpr int int_cw(int LA, int LB) {
   const int L = LA + LB;
   return L == 0 ? SNK_CW_L0 : L == 1 ? SNK_CW_L1 : L == 2 ? SNK_CW_L2 : L == 3 ? SNK_CW_L3 : L == 4 ? SNK_CW_L4 : L == 5 ? SNK_CW_L5 : SNK_CW_L6;
 }
-__host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_cw(LA, LB) + 32; }
+__host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_cw(LA, LB); }
 
-#ifndef SNK_NS_LB0
-#define SNK_NS_LB0 8
+// depth of a warp's prefetch ring (a power of two): units in flight ahead of the one being evaluated
+#ifndef SNK_D_L0
+#define SNK_D_L0 8
 #endif
-#ifndef SNK_NS_LB1
-#define SNK_NS_LB1 8
+#ifndef SNK_D_L1
+#define SNK_D_L1 4
 #endif
-__host__ __device__ constexpr int int_nslots(int LA, int LB) { return (LA + LB >= 4 ? 4 : LB == 0 ? SNK_NS_LB0 : LB == 1 ? SNK_NS_LB1 : 8) * int_cw(LA, LB) / 4; }
-__host__ __device__ constexpr int int_slot_bytes(int LB) { return kUnitBytes + ncart(LB) * kTile * 8; }
-// ring slots, then full[NS] and empty[NS] mbarriers, then the per-group unit counters and the unit count
-__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_nslots(LA, LB) * int_slot_bytes(LB) + 2 * 8 * int_nslots(LA, LB) + 32; }
+#ifndef SNK_D_L2
+#define SNK_D_L2 4
+#endif
+#ifndef SNK_D_LHI
+#define SNK_D_LHI 2
+#endif
+__host__ __device__ constexpr int int_depth(int LA, int LB) { return LA + LB == 0 ? SNK_D_L0 : LA + LB == 1 ? SNK_D_L1 : LA + LB == 2 ? SNK_D_L2 : SNK_D_LHI; }
+// one ring slot of a warp: the unit record, then ncart(l_b) row segments of F for the 32 NP points of the warp
+__host__ __device__ constexpr int int_slot_bytes(int LB, int NP) { return kUnitBytes + ncart(LB) * 32 * NP * 8; }
+// per warp: D slots; then D full-mbarriers per warp
+__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) {
+  return int_cw(LA, LB) * int_depth(LA, LB) * (int_slot_bytes(LB, int_npmax(LA, LB)) + 8);
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -160,13 +172,24 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                : "memory");
 }
 
-// ---- consumer side: this warp's share of the unit stream for the points [pbase, pbase + 32 NP) of the tile, NP per thread ----
-// s_next: shared counter of the warp's point group (next unit nobody of the group has taken); nunit: units of the tile's stream.
-template <int LA, int LB, int NP>
-__device__ __forceinline__ void consume_units(const IntParams& p, const unsigned char* smem_int, uint32_t s_full, uint32_t s_empty,
-                                              int* s_next, int nunit, const TileRec& tile, int64_t col0, int pbase, int lane) {
+// ---- one warp: its share (entries rnk, rnk + WPG, ... of the list) of the tile's unit stream for the points
+// [pbase, pbase + 32 NP) of the tile, NP per thread ----
+template <int LA, int LB, int NP, int WPG>
+__device__ __forceinline__ void consume_units(const IntParams& p, const TileRec& tile, const int32_t* __restrict__ list, int cnt,
+                                              unsigned char* ring, uint32_t s_bar, int pbase, int rnk, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
-  constexpr int NS = int_nslots(LA, LB), SLOT = int_slot_bytes(LB);
+  constexpr int D = int_depth(LA, LB), SLOT = int_slot_bytes(LB, int_npmax(LA, LB));
+  constexpr uint32_t FROW = 32u * NP * 8u;             // bytes of one staged F row segment
+  const int n_my = cnt > rnk ? (cnt - rnk + WPG - 1) / WPG : 0;
+  if (n_my == 0) return;
+  const uint32_t s_ring = smem_u32(ring);
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < D; ++i) mbar_init(s_bar + 8 * i, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncwarp();
+
   int pt[NP], ptc[NP];
   bool act[NP];
   double gx[NP], gy[NP], gz[NP];
@@ -178,9 +201,39 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
     const int64_t slot = tile.slot + ptc[s];
     gx[s] = p.gx[slot]; gy[s] = p.gy[slot]; gz[s] = p.gz[slot];
   }
+  const int64_t col0 = tile.slot - p.slot0;
   const double* __restrict__ Fc = p.F + col0;
   double* __restrict__ Gc = p.G + col0;
   const int64_t ld = p.ld;
+
+  // unit ids and (fb | nprim << 24) of this warp's units [32 w, 32 w + 32): lane i holds unit 32 w + i; two windows in flight
+  auto load_win = [&](int wb, int& e, int& m) {
+    const int q = wb + lane;
+    e = 0; m = 0;
+    if (q < n_my) {
+      e = __ldg(list + (int64_t)q * WPG + rnk);
+      const int2 mm = __ldg(reinterpret_cast<const int2*>(&p.meta[e].fb));   // fb, nprim | first << 8
+      m = mm.x | (mm.y & 0xff) << 24;
+    }
+  };
+  // stage this warp's k-th unit into slot k % D
+  auto issue = [&](int k, int e_w, int m_w) {
+    const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
+    if (lane == 0) {
+      const uint32_t slot = (uint32_t)k % D, bar = s_bar + 8 * slot, dst = s_ring + slot * SLOT;
+      const uint32_t nb = 64u + ((uint32_t)m >> 24) * (uint32_t)kPrimBytes;
+      // (the slot was only READ through the generic proxy, and every lane's reads precede the __syncwarp: no proxy fence needed)
+      mbar_arrive_expect_tx(bar, nb + NB * FROW);
+      bulk_g2s(dst, p.units + (size_t)e * kUnitBytes, nb, bar);
+      const double* __restrict__ Fsrc = Fc + (int64_t)(m & 0xffffff) * ld + pbase;
+#pragma unroll
+      for (int k2 = 0; k2 < NB; ++k2) bulk_g2s(dst + kUnitBytes + k2 * FROW, Fsrc + (int64_t)k2 * ld, FROW, bar);
+    }
+  };
+  int e0, m0, e1, m1;
+  load_win(0, e0, m0);
+  load_win(32, e1, m1);
+  for (int k = 0; k < D && k < n_my; ++k) issue(k, e0, m0);
 
   int cur_fa = -1;
   int64_t cur_offa = 0;
@@ -199,21 +252,18 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
       }
   };
 
-  auto take = [&]() {                                  // next unit of the group's stream
-    int u = 0;
-    if (lane == 0) u = atomicAdd(s_next, 1);
-    return __shfl_sync(0xffffffffu, u, 0);
-  };
-  int u = take();
-  while (u < nunit) {
-    const uint32_t sl = (uint32_t)u % NS, phase = ((uint32_t)u / NS) & 1u;
-    if (!mbar_test(s_full + 8 * sl, phase)) mbar_wait(s_full + 8 * sl, phase);
-    const int unext = take();                          // the shared-memory round trip overlaps this unit's recurrences
-    const unsigned char* rec = smem_int + sl * SLOT;
+#pragma unroll 1
+  for (int k = 0; k < n_my; ++k) {
+    const uint32_t sl = (uint32_t)k % D, phase = ((uint32_t)k / D) & 1u;
+    if (!mbar_test(s_bar + 8 * sl, phase)) mbar_wait(s_bar + 8 * sl, phase);
+    const unsigned char* rec = ring + sl * SLOT;
     const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
     const int fa = h0.x, fb = h0.y;
-    const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);   // ABx, ABy
-    const double ABz = *reinterpret_cast<const double*>(rec + 32);
+    double ABx = 0.0, ABy = 0.0, ABz = 0.0;
+    if constexpr (LB > 0) {
+      const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
+      ABx = ab0.x; ABy = ab0.y; ABz = *reinterpret_cast<const double*>(rec + 32);
+    }
     const longlong2 off = *reinterpret_cast<const longlong2*>(rec + 48);   // fa * ld, fb * ld
     if (fa != cur_fa) {
       if (cur_fa >= 0) flush_a();
@@ -228,123 +278,65 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const unsigned
 #pragma unroll
     for (int s = 0; s < NP; ++s)
 #pragma unroll
-      for (int k = 0; k < NB; ++k) { Fb[s][k] = Fs[k * kTile + ptc[s]]; Gb[s][k] = 0.0; }
+      for (int k2 = 0; k2 < NB; ++k2) { Fb[s][k2] = Fs[k2 * (32 * NP) + 32 * s + lane]; Gb[s][k2] = 0.0; }
 
     double acc[NP][nlev(LA, L)];
     theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
 #pragma unroll
     for (int s = 0; s < NP; ++s) {
       ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
-      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ab0.x, ab0.y, ABz, sink);
+      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ABx, ABy, ABz, sink);
     }
 
-    __syncwarp();
-    if (lane == 0) mbar_arrive(s_empty + 8 * sl);                  // slot may be refilled
+    __syncwarp();                                                  // every lane is done with the slot: refill it D units ahead
+    const int kn = k + D;
+    if (kn < n_my) {
+      if ((kn & 31) == 0) { e0 = e1; m0 = m1; load_win(kn + 32, e1, m1); }
+      issue(kn, e0, m0);
+    }
     if (fa != fb) {                                                // a == b (same shell): one direction only
 #pragma unroll
       for (int s = 0; s < NP; ++s)
         if (act[s]) {
 #pragma unroll
-          for (int k = 0; k < NB; ++k) atomicAdd(Gc + off.y + (int64_t)k * ld + pt[s], Gb[s][k]);
+          for (int k2 = 0; k2 < NB; ++k2) atomicAdd(Gc + off.y + (int64_t)k2 * ld + pt[s], Gb[s][k2]);
         }
     }
-    u = unext;
   }
   if (cur_fa >= 0) flush_a();
 }
 
 template <int LA, int LB>
 __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_integrals(IntParams p) {
-  constexpr int NB = ncart(LB);
-  constexpr int NPM = int_npmax(LA, LB), CW = int_cw(LA, LB);       // points per thread, consumer warps per CTA
-  constexpr int WPG = CW * NPM * 32 / kTile;                         // consumer warps per point group
-  static_assert(WPG >= 1 && WPG * (kTile / (32 * NPM)) == CW, "consumer warps: a whole number per point group");
-  constexpr int NS = int_nslots(LA, LB), NG = NS / 2, SLOT = int_slot_bytes(LB);
+  constexpr int NPM = int_npmax(LA, LB), CW = int_cw(LA, LB);       // points per thread, warps per CTA
+  constexpr int WPG = CW * NPM * 32 / kTile;                         // warps per point group
+  static_assert(WPG >= 1 && WPG * (kTile / (32 * NPM)) == CW, "warps: a whole number per point group");
+  constexpr int D = int_depth(LA, LB), SLOT = int_slot_bytes(LB, NPM);
+  static_assert((D & (D - 1)) == 0, "ring depth");
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
-  const uint32_t s_base = smem_u32(smem_int);
-  const uint32_t s_full = s_base + NS * SLOT, s_empty = s_full + NS * 8;
-  int* s_ctr = reinterpret_cast<int*>(smem_int + NS * SLOT + 16 * NS);   // [0..3] next unit of point group g, [4] units of the tile
 
   const TileRec tile = p.tiles[blockIdx.x];
-  const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
-  const uint32_t* __restrict__ mask = p.vmask + (int64_t)tile.batch * p.vstride;
-  const int w0 = p.pbeg >> 5, w1 = (p.pend + 31) >> 5;
-  auto class_bits = [&](int w) {                           // V_j bits of word w that belong to this class
-    uint32_t word = __ldg(mask + w);
-    if (w == w0) word &= 0xffffffffu << (p.pbeg & 31);
-    if (w == w1 - 1 && (p.pend & 31)) word &= 0xffffffffu >> (32 - (p.pend & 31));
-    return word;
-  };
-  // length of the tile's unit stream
-  int cnt = 0;
-  for (int w = w0 + t; w < w1; w += int_threads(LA, LB)) cnt += __popc(class_bits(w));
-  cnt = __reduce_add_sync(0xffffffffu, cnt);
-  if (t < 8) s_ctr[t] = 0;
-  __syncthreads();
-  if (lane == 0 && cnt) atomicAdd(s_ctr + 4, cnt);
-  const int nag = (tile.n + 32 * NPM - 1) / (32 * NPM);    // point groups that own at least one point
-  if (t == 0) {
-    for (int i = 0; i < NS; ++i) { mbar_init(s_full + 8 * i, 1); mbar_init(s_empty + 8 * i, nag); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  const int nunit = s_ctr[4];
-  if (nunit == 0) return;
-  const int64_t col0 = tile.slot - p.slot0;
-
-  if (warp == CW) {
-    // ------------------------------------------------ producer warp ------------------------------------------------
-    const int npad = ((tile.n + 31) >> 5) << 5;
-    const uint32_t frow = (uint32_t)npad * 8u;             // bytes of one staged F row
-    uint32_t u = 0;                                        // units issued so far
-    for (int wb = w0; wb < w1; wb += 32) {
-      const int w = wb + lane;
-      const uint32_t word = w < w1 ? class_bits(w) : 0u;
-      uint32_t any = __ballot_sync(~0u, word != 0u);
-      while (any) {
-        const int src = __ffs(any) - 1;
-        any &= any - 1;
-        const uint32_t bits = __shfl_sync(~0u, word, src);
-        const int n = __popc(bits);
-        const int base_pid = (wb + src) << 5;
-        for (int b0 = 0; b0 < n; b0 += NG) {               // NG units per step (half the ring): one lane per unit
-          const int cnt_step = min(n, b0 + NG) - b0;
-          if (lane >= b0 && lane < b0 + cnt_step) {
-            const int pid = base_pid + (int)__fns(bits, 0, lane + 1);
-            const UnitMeta m = p.meta[pid];                // in flight while we wait for the slot
-            const uint32_t uu = u + (uint32_t)(lane - b0), slot = uu % NS;
-            // the slot's previous unit is released by the one warp of every point group that processed it
-            if (uu >= NS) mbar_wait_suspend(s_empty + 8 * slot, (uu / NS - 1) & 1);
-            const uint32_t nb = 64u + (uint32_t)(m.nprim_first & 0xff) * (uint32_t)kPrimBytes;
-            const uint32_t bar = s_full + 8 * slot, dst = s_base + slot * SLOT;
-            mbar_arrive_expect_tx(bar, nb + NB * frow);
-            bulk_g2s(dst, p.units + (size_t)pid * kUnitBytes, nb, bar);
-            const double* __restrict__ Fsrc = p.F + (int64_t)m.fb * p.ld + col0;
-#pragma unroll
-            for (int k = 0; k < NB; ++k) bulk_g2s(dst + kUnitBytes + k * (kTile * 8), Fsrc + (int64_t)k * p.ld, frow, bar);
-          }
-          u += (uint32_t)cnt_step;
-          __syncwarp();
-        }
-      }
-    }
-    return;
-  }
-  const int grp = warp / WPG, pbase = grp * 32 * NPM;
+  const int jj = tile.batch - p.b0;
+  const int cnt = p.vcnt[jj * kNumClasses + p.cls];                  // units of this class kept by the tile's batch
+  if (cnt == 0) return;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int grp = warp / WPG, rnk = warp % WPG, pbase = grp * 32 * NPM;
   if (pbase >= tile.n) return;
+  const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg;
+  unsigned char* ring = smem_int + warp * (D * SLOT);
+  const uint32_t s_bar = smem_u32(smem_int + CW * D * SLOT) + warp * (D * 8);
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
-  int* s_next = s_ctr + grp;
   if constexpr (NPM == 4) {
-    if (need == 4) consume_units<LA, LB, 4>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
-    else if (need == 3) consume_units<LA, LB, 3>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
-    else if (need == 2) consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
-    else consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    if (need == 4) consume_units<LA, LB, 4, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    else if (need == 3) consume_units<LA, LB, 3, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    else if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
   } else if constexpr (NPM == 2) {
-    if (need == 2) consume_units<LA, LB, 2>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
-    else consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
   } else {
-    consume_units<LA, LB, 1>(p, smem_int, s_full, s_empty, s_next, nunit, tile, col0, pbase, lane);
+    consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
   }
 }
 

@@ -96,7 +96,10 @@ struct IntParams {
   int64_t ld;              // leading dimension of F/G (slots of the super-batch, padded)
   int64_t slot0;           // first slot of the super-batch
   const TileRec* tiles; int ntiles;
-  const uint32_t* vmask; int64_t vstride;   // words per batch
+  const int32_t* vlist; int64_t vlstride;   // kept unit ids of the super-batch's batches (k_vlist), ints per batch row
+  const int32_t* vcnt;                      // [batches of the super-batch][kNumClasses] kept units per class
+  int b0;                                   // first batch of the super-batch
+  int cls;                                  // class of this launch
   int pbeg, pend;          // range of this class in the unit list
   const unsigned char* units;               // [nunit][kUnitBytes]
   const UnitMeta* meta;                     // [nunit]

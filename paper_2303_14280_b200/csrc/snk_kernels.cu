@@ -374,8 +374,9 @@ __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict_
 // V_j bit masks (Eq. 43): one thread per (batch, unit); every unit of a pair takes the pair's decision
 __global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const double* __restrict__ FtsT, int nshld,
                         const double* __restrict__ phit, double eps, uint32_t* __restrict__ vmask, int64_t vstride) {
-  const int j = blockIdx.x;
-  const int i = blockIdx.y * blockDim.x + threadIdx.x;
+  const int nblk_u = (nunit + 255) / 256;            // flattened grid: the batch index may exceed grid.y's 65535
+  const int j = blockIdx.x / nblk_u;
+  const int i = (blockIdx.x % nblk_u) * blockDim.x + threadIdx.x;
   bool keep = false;
   if (i < nunit) {
     const UnitMeta m = meta[i];
@@ -386,6 +387,51 @@ __global__ void k_vmask(int nunit, const UnitMeta* __restrict__ meta, const doub
   }
   const unsigned bal = __ballot_sync(~0u, keep);
   if ((threadIdx.x & 31) == 0 && (i >> 5) < vstride) vmask[(int64_t)j * vstride + (i >> 5)] = bal;
+}
+
+// Unit lists of the batches [b0, b0 + nb) for the integral kernel: the set bits of V_j, class by class, as unit ids.
+// list[(j - b0) * stride + cls_beg[c] + q] = q-th kept unit of class c in batch j (ascending: the (a, b) order of the unit table),
+// cnt[(j - b0) * kNumClasses + c] = their number.  The slot of a class inside a batch's row is as long as the class itself, so no
+// offsets have to be scanned and nothing has to be sized on the host.  One CTA per batch.
+struct ClassBeg { int v[kNumClasses + 1]; };
+__global__ void __launch_bounds__(256) k_vlist(int b0, ClassBeg cb, const uint32_t* __restrict__ vmask, int64_t vstride,
+                                               int32_t* __restrict__ list, int64_t stride, int32_t* __restrict__ cnt) {
+  __shared__ int wsum[8];
+  const int jj = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const uint32_t* __restrict__ mrow = vmask + (int64_t)(b0 + jj) * vstride;
+  int32_t* __restrict__ out_b = list + (int64_t)jj * stride;
+  for (int c = 0; c < kNumClasses; ++c) {
+    const int pbeg = cb.v[c], pend = cb.v[c + 1];
+    int running = 0;
+    if (pend > pbeg) {
+      const int w0 = pbeg >> 5, w1 = (pend + 31) >> 5;
+      int32_t* __restrict__ out = out_b + pbeg;
+      for (int wb = w0; wb < w1; wb += 256) {
+        const int w = wb + t;
+        uint32_t word = 0u;
+        if (w < w1) {
+          word = mrow[w];
+          if (w == w0) word &= 0xffffffffu << (pbeg & 31);
+          if (w == w1 - 1 && (pend & 31)) word &= 0xffffffffu >> (32 - (pend & 31));
+        }
+        const int n = __popc(word);
+        int inc = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(~0u, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        int base = 0, total = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { const int v = wsum[k]; if (k < warp) base += v; total += v; }
+        int o = running + base + inc - n;
+        const int id0 = w << 5;
+        while (word) { const int b = __ffs(word) - 1; word &= word - 1; out[o++] = id0 + b; }
+        running += total;
+        __syncthreads();
+      }
+    }
+    if (t == 0) cnt[jj * kNumClasses + c] = running;
+  }
 }
 
 // counters for snk_stats: out[0]=sum|V_j|, [1]=pair-points, [2]=contracted integrals, [3]=primitive integrals,
@@ -597,8 +643,19 @@ cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t*
 cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
                       uint32_t* vmask, int64_t vstride, cudaStream_t s) {
   if (nbatch > 0 && nunit > 0) {
-    dim3 g((unsigned)nbatch, nblk(nunit, 256));
-    k_vmask<<<g, 256, 0, s>>>(nunit, meta, FtsT, nshld, phit, eps, vmask, vstride);
+    const int64_t nb = (int64_t)nbatch * nblk(nunit, 256);
+    if (nb > 0x7fffffff) return cudaErrorInvalidConfiguration;
+    k_vmask<<<(unsigned)nb, 256, 0, s>>>(nunit, meta, FtsT, nshld, phit, eps, vmask, vstride);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t run_vlist(int b0, int nb, const int* cls_beg, const uint32_t* vmask, int64_t vstride, int32_t* list, int64_t stride,
+                      int32_t* cnt, cudaStream_t s) {
+  if (nb > 0) {
+    ClassBeg cb;
+    for (int c = 0; c <= kNumClasses; ++c) cb.v[c] = cls_beg[c];
+    k_vlist<<<(unsigned)nb, 256, 0, s>>>(b0, cb, vmask, vstride, list, stride, cnt);
   }
   return cudaGetLastError();
 }

@@ -42,6 +42,8 @@ cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t*
                           UnitMeta* meta, cudaStream_t s);
 cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
                       uint32_t* vmask, int64_t vstride, cudaStream_t s);
+cudaError_t run_vlist(int b0, int nb, const int* cls_beg, const uint32_t* vmask, int64_t vstride, int32_t* list, int64_t stride,
+                      int32_t* cnt, cudaStream_t s);
 cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
                        int64_t vstride, const double* cfp, const double* cfc, double* out, cudaStream_t s);
 cudaError_t run_colloc(const ShellTab& sh, const TileRec* tiles, int ntiles, const double* gx, const double* gy, const double* gz,
