@@ -128,7 +128,7 @@ def run_reference(args, rank, world):
         return
     from oracle import oracle as orc
     from paper_2303_14280_b200 import inputs
-    w = inputs.make_workload(args.config, grid=args.grid, device=_gen_device())
+    w = inputs.make_workload(args.config, grid=args.grid, device=_gen_device(), density=args.density)
     first = time_oracle_sample(w, target_s=args.cpu_seconds, return_idx=True)
     idx = first.pop("idx")
     o = orc.Oracle(w.basis)
@@ -148,7 +148,7 @@ def run_reference(args, rank, world):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args.config, w), "sample": sample, "batch_cell": w.batch_cell, "batch_max": w.batch_max},
+            "config": {"workload": _workload_name(args.config, w), "sample": sample, "density": args.density, "batch_cell": w.batch_cell, "batch_max": w.batch_max},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": st["threads"], "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -195,6 +195,9 @@ def main():
                          "(1 029 atoms) takes minutes per build and is run with --config 4 --steps 1")
     ap.add_argument("--grid", type=lambda s: tuple(int(x) for x in s.split(",")), default=None, help="override n_r,n_theta,n_phi")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--density", default="dense", choices=["dense", "decay"],
+                    help="'dense' = BASELINE.json's P = C C^T with Gaussian C (no spatial decay: V_j keeps every significant pair); "
+                         "'decay' = localised random orbitals, |P| ~ exp(-r / 1.5 bohr) (SURVEY.md section 8(f)-2: sn-LinK deletes work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--workspace-gb", type=float, default=None)
@@ -225,9 +228,9 @@ def main():
     snk.load()
 
     # ---- synthetic workload (seeded, DESIGN.md recipe); the grid generator runs on the GPU for speed ----
-    w = inputs.make_workload(args.config, grid=args.grid, device=str(dev))
+    w = inputs.make_workload(args.config, grid=args.grid, device=str(dev), density=args.density)
     shard = world > 1 and args.multi == "shard"
-    mine = shard_points(w.points, w.batch_cell, rank, world) if shard else np.ones(w.points.shape[0], dtype=bool)
+    mine = np.ones(w.points.shape[0], dtype=bool)
     if world > 1 and not shard:       # independent problem per rank: its own density matrix, same molecule and grid
         rng = np.random.Generator(np.random.PCG64(inputs.SEED_BASE + 1000 * rank + args.config))
         C = rng.standard_normal((w.basis.nbf, max(1, w.basis.nbf // 5))) / np.sqrt(max(1, w.basis.nbf // 5))
@@ -241,6 +244,17 @@ def main():
     if args.workspace_gb:
         s.set_option("workspace_gb", args.workspace_gb)
     dfma_peak, dmma_peak = snk.measure_fp64_peak(5)
+    if shard:
+        # Alg. 2 on the library's own work model: one screening pass over the whole grid gives the primitive
+        # pair-points of every batch; root cells are dealt to ranks by greedy LPT on them (replicated, deterministic)
+        from paper_2303_14280_b200.dist import root_cell_costs
+        s.set_grid(pts, wts)
+        s.screen(P)
+        L = s.export_lists(want_V=False)
+        cells = root_cell_costs(w.points, w.batch_cell, L["batch_off"], L["perm"], s.batch_costs())
+        mine = shard_points(w.points, w.batch_cell, rank, world, cell_costs=cells)
+        pts = torch.as_tensor(np.ascontiguousarray(w.points[mine]), device=dev)
+        wts = torch.as_tensor(np.ascontiguousarray(w.weights[mine]), device=dev)
     s.set_grid(pts, wts)
     set_grid_ms = s.stats()["ms_set_grid"]
 
@@ -319,6 +333,10 @@ def main():
                 "all_integral_kernels": {"achieved": st["flops_integral"] / (all_ms * 1e-3) * 1e-12 if all_ms > 0 else 0.0, "ms": all_ms,
                                          "flops": st["flops_integral"], "share_of_step": all_ms / st["ms_build"] if st["ms_build"] else None},
                 "gemm_dmma": {"peak": dmma_peak, "achieved": st["flops_gemm"] / ((st["ms_F"] + st["ms_Kt"] + 1e-12) * 1e-3) * 1e-12,
+                              "achieved_algorithmic": st["flops_gemm_alg"] / ((st["ms_F"] + st["ms_Kt"] + 1e-12) * 1e-3) * 1e-12,
+                              "flops_executed": st["flops_gemm"], "flops_algorithmic": st["flops_gemm_alg"],
+                              "note": "executed = row lists of the chunks padded to the 16 / 32 wide tiles (plus the small screening GEMM); "
+                                      "algorithmic = 2 |Q_j| nbf(B_j) nbf per batch for a4 and for a6 (Eq. 48 operand sizes)",
                               "ms_F": st["ms_F"], "ms_Kt": st["ms_Kt"]},
                 "per_class": {snk.CLASS_NAMES[c]: {"ms": st["ms_G_class"][c], "achieved": st["flops_class"][c] / (st["ms_G_class"][c] * 1e-3) * 1e-12,
                                                    "frac": st["flops_class"][c] / (st["ms_G_class"][c] * 1e-3) * 1e-12 / dfma_peak if dfma_peak else None}
@@ -333,7 +351,9 @@ def main():
                                           "summary under profiles/",
                        "l2": "working set (Phi, F, G slabs) far larger than the 126 MB L2; no flush needed",
                        "parallelism": "1 GPU" if world == 1 else ("root cells -> %d ranks by Alg. 2 LPT, NCCL all-reduce of K per build" % world if shard else "%d independent replicas (own density each), no collective" % world),
-                       "batch_cell": w.batch_cell, "batch_max": w.batch_max, "n_int_per_step": n_int, "n_int_primitive_per_step": n_prim,
+                       "batch_cell": w.batch_cell, "batch_max": w.batch_max, "density": args.density,
+                       "pair_survival": (st["sum_V"] / (st["nbatch"] * st["npair_sig"])) if st["nbatch"] and st["npair_sig"] else None,
+                       "n_int_per_step": n_int, "n_int_primitive_per_step": n_prim,
                        "n_pairpoints_per_step": n_pp},
             "clocks": clocks,
             "e2e": {"value": n_int * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,

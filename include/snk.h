@@ -56,7 +56,7 @@ typedef struct snk_stats {
   double n_int_contracted;  /* sum_j |Q_j| sum_{(a,b) in V_j} ncart(l_a) ncart(l_b)  -- "integrals"  */
   double n_int_primitive;   /* same, times the number of primitive pairs actually evaluated          */
   double flops_integral;    /* FP64 flop model of the integral-contraction kernels */
-  double flops_gemm;        /* 2*M*N*K of the F and Kt contractions as executed                      */
+  double flops_gemm;        /* 2*M*N*K of the F and Kt contractions as executed (lists padded to tiles) */
   double ms_set_grid;       /* a0 + a1 + maxima                                                      */
   double ms_screen;         /* a3: |P|, Ftilde GEMM, V_j masks, pair tables                          */
   double ms_colloc;         /* a2                                                                    */
@@ -69,6 +69,7 @@ typedef struct snk_stats {
   double n_int_class[10];   /* contracted integrals per class                                        */
   double flops_class[10];   /* flop model per class                                                  */
   int64_t n_launches;       /* kernels of this library launched by the last snk_build_K              */
+  double flops_gemm_alg;    /* 2 |Q_j| nbf(B_j) nbf summed over batches, for a4 and a6 (Eq. 48 operands) */
 } snk_stats;
 
 /* ---- snk_create: the basis set "B" of Alg. 1 -------------------------------------
@@ -111,6 +112,15 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream);
 /* Same build with HOST buffers: H2D copy of P, build, D2H copy of K, stream synchronised on return.
  * This is the end-to-end call bench.py times as "e2e". */
 int snk_build_K_host(snk_ctx* ctx, const double* P_host, double* K_host, void* stream);
+
+/* ---- work estimates for the batch-to-rank partition of Alg. 2 (cost model W_j, Eq. 49 at PAPER.md:330) --
+ * snk_screen runs only the density-dependent screening of snk_build_K (row a3, Eqs. 43-47: V_j for this P on the current
+ * grid), ordered on `stream`.  snk_batch_costs then returns, for every batch j in batch order,
+ *   cost[j] = |Q_j| * (primitive pairs of the shell pairs kept in V_j)     -- primitive pair-points, what a5's time follows.
+ *   P DEVICE [nbf*nbf]     cost HOST [nbatch] (nbatch from snk_get_stats / snk_export_lists); synchronises the stream.
+ * Errors: SNK_ESTATE before snk_set_grid / before a screening or build. */
+int snk_screen(snk_ctx* ctx, const double* P, void* stream);
+int snk_batch_costs(snk_ctx* ctx, double* cost);
 
 /* sum over shells of (l+1)(l+2)/2 */
 int snk_nbf(const snk_ctx* ctx);

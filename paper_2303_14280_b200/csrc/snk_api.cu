@@ -20,7 +20,7 @@ using namespace snk;
 namespace {
 thread_local std::string g_create_error;
 
-struct Super { int b0, b1; int64_t slot0, nslots; int t0, t1; int64_t f0; };   // f0: first 128-column tile (a4 activity bits)
+struct Super { int b0, b1; int64_t slot0, nslots; int t0, t1; int c0, c1, ct0, ct1, max_nrow; };   // batches, tiles, chunks, a4 column tiles
 
 enum Stage { ST_SCREEN = 0, ST_COLLOC, ST_F, ST_G, ST_KT, ST_SYM, ST_COUNT };
 }  // namespace
@@ -47,17 +47,18 @@ struct snk_ctx {
   DevBuf<uint32_t> d_bmask;
   DevBuf<unsigned long long> d_phimax, d_Fmax;
   DevBuf<TileRec> d_tiles;
-  DevBuf<uint32_t> d_act;       // a6: activity bits of Phi blocks (row tile x 16-slot k-tile)
-  int64_t actw = 0;
-  DevBuf<uint32_t> d_actF;      // a4: activity bits of Phi blocks (128-slot column tile x 16-function k-tile)
-  int kwordsF = 0;
+  DevBuf<ChunkRec> d_chunks;    // a4 / a6: chunks of whole batches, their row lists L (functions in the union of B_j)
+  DevBuf<int32_t> d_rowlist, d_nrows;
+  DevBuf<ColTile> d_ctiles;     // a4: 128-slot column tiles of the chunks
+  int64_t lstride = 0;
+  double flops_gemm_alg = 0.0;  // 2 |Q_j| nbf(B_j) nbf per contraction, summed over the batches (Eq. 48's operand sizes)
   std::vector<int32_t> h_bn;
   std::vector<int64_t> h_bslot;
   std::vector<TileRec> h_tiles;
   std::vector<Super> supers;
   DevBuf<double> d_Phi, d_F, d_G;
   // build state
-  bool have_build = false, stats_valid = false;
+  bool have_build = false, have_screen = false, stats_valid = false;
   DevBuf<double> d_absP, d_Ftf, d_FtsT, d_Kt, d_Pin, d_Kout, d_stats, d_cflops;
   DevBuf<int32_t> d_flag, d_np, d_pos, d_ppos;     // per candidate pair: #units, is-pair flag, and their exclusive scans
   DevBuf<unsigned char> d_units;                    // [nunit][kUnitBytes]
@@ -274,7 +275,8 @@ void snk_destroy(snk_ctx* ctx) {
   ctx->d_poff.release(); ctx->d_nprim.release(); ctx->d_lshells.release();
   ctx->gx.release(); ctx->gy.release(); ctx->gz.release(); ctx->gw.release(); ctx->d_PhiTf.release(); ctx->d_phit.release();
   ctx->slot_src.release(); ctx->d_bslot.release(); ctx->d_bn.release(); ctx->d_bmask.release(); ctx->d_phimax.release();
-  ctx->d_Fmax.release(); ctx->d_tiles.release(); ctx->d_act.release(); ctx->d_actF.release(); ctx->d_Phi.release(); ctx->d_F.release(); ctx->d_G.release();
+  ctx->d_Fmax.release(); ctx->d_tiles.release(); ctx->d_chunks.release(); ctx->d_rowlist.release(); ctx->d_nrows.release();
+  ctx->d_ctiles.release(); ctx->d_Phi.release(); ctx->d_F.release(); ctx->d_G.release();
   ctx->d_absP.release(); ctx->d_Ftf.release(); ctx->d_FtsT.release(); ctx->d_Kt.release();
   ctx->d_Pin.release(); ctx->d_Kout.release(); ctx->d_stats.release(); ctx->d_cflops.release();
   ctx->d_flag.release(); ctx->d_np.release(); ctx->d_pos.release(); ctx->d_ppos.release(); ctx->d_units.release();
@@ -334,6 +336,7 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
     }
   ctx->cand.off[kNumClasses] = off;
   if (off >= (int64_t)1 << 31) return bail(SNK_EINVAL, "snk_create: too many shells (candidate pairs exceed 2^31)");
+  if (nshells > 65535) return bail(SNK_EINVAL, "snk_create: more than 65535 shells (grid.y of the per-shell screening kernels)");
 
   cudaError_t e = cudaSuccess;
   auto up = [&](auto& buf, const auto& vec) { if (e == cudaSuccess) e = upload(buf, vec); };
@@ -484,6 +487,8 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
     }
     ctx->nbatch = (int)ctx->h_bn.size();
     ctx->nslots = slot;
+    for (int n : ctx->h_bn)      // k_maxima holds a batch in 16 x 256 registers; only > 4096 coincident points at depth 20 get here
+      if (n > 4096) FAIL(SNK_EINVAL, "snk_set_grid: a batch holds more than 4096 points (coincident points beyond octree depth 20)");
     const int nb = ctx->nbatch;
     if (nb > 0) {
       DevBuf<int64_t> d_bsrc_begin;
@@ -496,21 +501,6 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       CK(ctx->gx.reserve(slot)); CK(ctx->gy.reserve(slot)); CK(ctx->gz.reserve(slot)); CK(ctx->gw.reserve(slot)); CK(ctx->slot_src.reserve(slot));
       CK(run_fill_slots(nb, d_bsrc_begin.p, ctx->d_bn.p, ctx->d_bslot.p, idx2.p, points, weights, ctx->gx.p, ctx->gy.p, ctx->gz.p,
                         ctx->gw.p, ctx->slot_src.p, s));
-      ctx->actw = (slot / 16 + 31) / 32 + 1;
-      CK(ctx->d_act.reserve((size_t)((ctx->nbf + kt_row_tile() - 1) / kt_row_tile()) * ctx->actw));
-      CK(run_kt_flags(ctx->tab(), nb, ctx->d_bn.p, ctx->d_bslot.p, ctx->d_bmask.p, ctx->nshw, ctx->d_act.p, ctx->actw, s));
-      {   // executed a6 flops: 2 * rows of the tile * 16 * nbf per set bit
-        const int nmt = (ctx->nbf + kt_row_tile() - 1) / kt_row_tile();
-        std::vector<uint32_t> ha((size_t)nmt * ctx->actw);
-        CK(cudaMemcpyAsync(ha.data(), ctx->d_act.p, ha.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));
-        ctx->flops_Kt = 0.0;
-        for (int mt = 0; mt < nmt; ++mt) {
-          int64_t bits = 0;
-          for (int64_t i = 0; i < ctx->actw; ++i) bits += __builtin_popcount(ha[(size_t)mt * ctx->actw + i]);
-          ctx->flops_Kt += 2.0 * std::min(kt_row_tile(), ctx->nbf - kt_row_tile() * mt) * 16.0 * ctx->nbf * (double)bits;
-        }
-      }
       // ---- Eq. 47 maxima (density independent) ----
       ctx->ldj = (nb + 7) / 8 * 8;
       CK(ctx->d_PhiTf.reserve((size_t)ctx->nbf * ctx->ldj)); CK(ctx->d_phit.reserve(nb));
@@ -522,9 +512,14 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
       std::vector<uint32_t> hm((size_t)nb * ctx->nshw);
       CK(cudaMemcpyAsync(hm.data(), ctx->d_bmask.p, hm.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
       CK(cudaStreamSynchronize(s));
-      for (int j = 0; j < nb; ++j)
+      ctx->flops_gemm_alg = 0.0;
+      for (int j = 0; j < nb; ++j) {
+        int64_t nf = 0;
         for (int a = 0; a < nsh; ++a)
-          if ((hm[(size_t)j * ctx->nshw + (a >> 5)] >> (a & 31)) & 1u) ctx->sum_B_fn += ncart(ctx->h_l[a]);
+          if ((hm[(size_t)j * ctx->nshw + (a >> 5)] >> (a & 31)) & 1u) nf += ncart(ctx->h_l[a]);
+        ctx->sum_B_fn += nf;
+        ctx->flops_gemm_alg += 2.0 * 2.0 * (double)ctx->h_bn[j] * (double)nf * ctx->nbf;      // a4 and a6
+      }
       // ---- tiles and super-batches (Alg. 1 line 8: as many batches as fit the workspace) ----
       for (int j = 0; j < nb; ++j)
         for (int o = 0; o < ctx->h_bn[j]; o += kTile)
@@ -553,34 +548,43 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
           return (double)x.n * h_bcnt[x.batch] * h_bcnt[x.batch] > (double)y.n * h_bcnt[y.batch] * h_bcnt[y.batch];
         });
       CK(upload(ctx->d_tiles, ctx->h_tiles));
-      {   // a4 activity bits (density independent)
-        std::vector<int64_t> h_bslot0(nb), h_btile0(nb);
-        int64_t f = 0;
+      {   // chunks of whole batches (<= kChunkSlots slots, never across super-batches), their row lists, a4 column tiles
+        std::vector<ChunkRec> h_chunks;
+        std::vector<ColTile> h_ct;
         for (Super& sp : ctx->supers) {
-          sp.f0 = f;
-          for (int j = sp.b0; j < sp.b1; ++j) { h_bslot0[j] = sp.slot0; h_btile0[j] = f; }
-          f += (sp.nslots + 127) / 128;
-        }
-        ctx->kwordsF = ((ctx->nbf + 15) / 16 + 31) / 32;
-        DevBuf<int64_t> d_bslot0, d_btile0;
-        CK(upload(d_bslot0, h_bslot0)); CK(upload(d_btile0, h_btile0));
-        CK(ctx->d_actF.reserve((size_t)f * ctx->kwordsF));
-        CK(run_f_flags(ctx->tab(), nb, ctx->d_bn.p, ctx->d_bslot.p, d_bslot0.p, d_btile0.p, ctx->d_bmask.p, ctx->nshw, ctx->d_actF.p, f,
-                       ctx->kwordsF, s));
-        {   // executed a4 flops: 2 * nbf * (functions of the k-tile) * (columns of the tile) per set bit
-          std::vector<uint32_t> hf((size_t)f * ctx->kwordsF);
-          CK(cudaMemcpyAsync(hf.data(), ctx->d_actF.p, hf.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-          CK(cudaStreamSynchronize(s));
-          ctx->flops_F = 0.0;
-          const int nkt = (ctx->nbf + 15) / 16;
-          for (const Super& sp : ctx->supers) {
-            const int64_t nt = (sp.nslots + 127) / 128;
-            for (int64_t tt = 0; tt < nt; ++tt) {
-              const double cw = (double)std::min<int64_t>(128, sp.nslots - 128 * tt);
-              for (int kt = 0; kt < nkt; ++kt)
-                if ((hf[(size_t)(sp.f0 + tt) * ctx->kwordsF + (kt >> 5)] >> (kt & 31)) & 1u)
-                  ctx->flops_F += 2.0 * ctx->nbf * std::min(16, ctx->nbf - 16 * kt) * cw;
+          sp.c0 = (int)h_chunks.size(); sp.ct0 = (int)h_ct.size();
+          for (int j = sp.b0; j < sp.b1;) {
+            ChunkRec ch; ch.slot0 = ctx->h_bslot[j]; ch.b0 = j; ch.pad = 0;
+            int64_t n = 0;
+            while (j < sp.b1) {
+              const int64_t pad = (ctx->h_bn[j] + kSlotAlign - 1) / kSlotAlign * kSlotAlign;
+              if (n > 0 && n + pad > kChunkSlots) break;
+              n += pad; ++j;
             }
+            ch.b1 = j; ch.nslots = (int32_t)n;
+            for (int64_t o = 0; o < n; o += 128) h_ct.push_back(ColTile{ch.slot0 + o, (int32_t)h_chunks.size(), (int32_t)std::min<int64_t>(128, n - o)});
+            h_chunks.push_back(ch);
+          }
+          sp.c1 = (int)h_chunks.size(); sp.ct1 = (int)h_ct.size();
+        }
+        const int nch = (int)h_chunks.size();
+        ctx->lstride = (ctx->nbf + 3) / 4 * 4;
+        CK(upload(ctx->d_chunks, h_chunks)); CK(upload(ctx->d_ctiles, h_ct));
+        CK(ctx->d_rowlist.reserve((size_t)nch * ctx->lstride)); CK(ctx->d_nrows.reserve(nch));
+        CK(run_chunk_rows(ctx->tab(), nch, ctx->d_chunks.p, ctx->d_bmask.p, ctx->nshw, ctx->d_rowlist.p, ctx->lstride, ctx->d_nrows.p, s));
+        std::vector<int32_t> h_nrows(nch);
+        CK(cudaMemcpyAsync(h_nrows.data(), ctx->d_nrows.p, (size_t)nch * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        // executed flops: a4 2 nbf (L padded to the k-tile) columns; a6 2 (L padded to the row tile) slots nbf
+        ctx->flops_F = ctx->flops_Kt = 0.0;
+        const int tk = f_k_tile(), ta = kt_row_tile();
+        for (Super& sp : ctx->supers) {
+          sp.max_nrow = 0;
+          for (int c = sp.c0; c < sp.c1; ++c) {
+            const int nr = h_nrows[c];
+            sp.max_nrow = std::max(sp.max_nrow, nr);
+            ctx->flops_F += 2.0 * ctx->nbf * (double)((nr + tk - 1) / tk * tk) * h_chunks[c].nslots;
+            ctx->flops_Kt += 2.0 * (double)((nr + ta - 1) / ta * ta) * h_chunks[c].nslots * ctx->nbf;
           }
         }
       }
@@ -603,21 +607,21 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
   });
 }
 
-int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
+static int build_impl(snk_ctx* ctx, const double* P, double* K, void* stream_, bool screen_only) {
   return guarded(ctx, [&]() -> int {
   if (!ctx) return SNK_EINVAL;
-  if (!P || !K) FAIL(SNK_EINVAL, "snk_build_K: NULL pointer");
+  if (!P || (!K && !screen_only)) FAIL(SNK_EINVAL, "snk_build_K: NULL pointer");
   CHECK_DEVICE();
   if (!ctx->have_grid) FAIL(SNK_ESTATE, "snk_build_K called before snk_set_grid");
   cudaStream_t s = (cudaStream_t)stream_;
   ctx->last_stream = s;
-  ctx->stats_valid = false; ctx->have_build = false;
+  ctx->stats_valid = false; ctx->have_build = false; ctx->have_screen = false;
   ctx->spans.clear(); ctx->ev_used = 0; ctx->gemm_flops = 0.0; ctx->n_launches = 0;
   const int nbf = ctx->nbf, nsh = ctx->nsh, nb = ctx->nbatch;
   const ShellTab tab = ctx->tab();
   CK(cudaEventRecord(ctx->ev_b0, s));
   if (nb == 0) {
-    CK(cudaMemsetAsync(K, 0, (size_t)nbf * nbf * sizeof(double), s));
+    if (K) CK(cudaMemsetAsync(K, 0, (size_t)nbf * nbf * sizeof(double), s));
     CK(cudaEventRecord(ctx->ev_b1, s));
     ctx->npair_sig = 0; ctx->nunit = 0; ctx->nprimpair = 0; ctx->have_build = true;
     return SNK_OK;
@@ -691,6 +695,12 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   ctx->n_launches += 6;
   span_end(sp);
   tr("screen", nunit, npair);
+  ctx->have_screen = true;
+  if (screen_only) {
+    CK(span_rc);
+    CK(cudaEventRecord(ctx->ev_b1, s));
+    return SNK_OK;
+  }
 
   CK(cudaMemsetAsync(ctx->d_Kt.p, 0, (size_t)nbf * nbf * sizeof(double), s));
   for (const Super& su : ctx->supers) {
@@ -703,7 +713,8 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     // ---- a4: F = P * Phi ----
     sp = span_begin(ST_F, -1);
     tr("colloc", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
-    CK(gemm_f(nbf, su.nslots, P, ctx->d_Phi.p, ctx->d_F.p, ctx->ld, ctx->d_actF.p + su.f0 * ctx->kwordsF, ctx->kwordsF, s));
+    CK(gemm_f(nbf, su.slot0, su.ct1 - su.ct0, ctx->d_ctiles.p + su.ct0, su.c0, ctx->d_nrows.p + su.c0,
+              ctx->d_rowlist.p + (int64_t)su.c0 * ctx->lstride, ctx->lstride, P, ctx->d_Phi.p, ctx->d_F.p, ctx->ld, s));
     span_end(sp);
     tr("F", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
     // ---- a5: G ----
@@ -728,7 +739,8 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
     span_end(sp);
     // ---- a6: Kt += Phi diag(w) G^T ----
     sp = span_begin(ST_KT, -1);
-    CK(gemm_kt(nbf, su.slot0, su.nslots, ctx->d_Phi.p, ctx->d_G.p, ctx->ld, ctx->gw.p, ctx->d_Kt.p, ctx->d_act.p, ctx->actw, s));
+    CK(gemm_kt(nbf, su.slot0, su.c1 - su.c0, su.max_nrow, ctx->d_chunks.p + su.c0, ctx->d_nrows.p + su.c0,
+               ctx->d_rowlist.p + (int64_t)su.c0 * ctx->lstride, ctx->lstride, ctx->d_Phi.p, ctx->d_G.p, ctx->ld, ctx->gw.p, ctx->d_Kt.p, s));
     ctx->n_launches += 3;   // collocation, F GEMM, Kt GEMM
     span_end(sp);
     tr("Kt", (int)(&su - ctx->supers.data()), (int)ctx->supers.size());
@@ -742,6 +754,28 @@ int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) {
   CK(span_rc);
   CK(cudaEventRecord(ctx->ev_b1, s));
   ctx->have_build = true;
+  return SNK_OK;
+  });
+}
+
+int snk_build_K(snk_ctx* ctx, const double* P, double* K, void* stream_) { return build_impl(ctx, P, K, stream_, false); }
+
+int snk_screen(snk_ctx* ctx, const double* P, void* stream_) { return build_impl(ctx, P, nullptr, stream_, true); }
+
+int snk_batch_costs(snk_ctx* ctx, double* cost) {
+  return guarded(ctx, [&]() -> int {
+  if (!ctx) return SNK_EINVAL;
+  if (!cost) FAIL(SNK_EINVAL, "snk_batch_costs: NULL pointer");
+  CHECK_DEVICE();
+  if (!ctx->have_grid || !ctx->have_screen) FAIL(SNK_ESTATE, "snk_batch_costs needs snk_set_grid and snk_screen / snk_build_K first");
+  cudaStream_t s = ctx->last_stream;
+  const int nb = ctx->nbatch;
+  if (nb == 0) return SNK_OK;
+  DevBuf<double> d;
+  CK(d.reserve(nb));
+  CK(run_batch_costs(nb, ctx->nunit, ctx->d_meta.p, ctx->d_bn.p, ctx->d_vmask.p, ctx->vstride, d.p, s));
+  CK(cudaMemcpyAsync(cost, d.p, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
   return SNK_OK;
   });
 }
@@ -792,6 +826,7 @@ int snk_get_stats(snk_ctx* ctx, snk_stats* out) {
     st.sum_V = (int64_t)h[0]; st.n_pairpoints = h[1]; st.n_int_contracted = h[2]; st.n_int_primitive = h[3];
     for (int c = 0; c < kNumClasses; ++c) { st.n_int_class[c] = h[4 + c]; st.flops_class[c] = h[16 + c]; }
     st.n_launches = ctx->n_launches;
+    st.flops_gemm_alg = ctx->flops_gemm_alg;
     st.flops_integral = h[14];
     double acc[ST_COUNT] = {0};
     for (int c = 0; c < kNumClasses; ++c) st.ms_G_class[c] = 0.0;

@@ -45,6 +45,14 @@ struct __align__(8) UnitMeta {
 };
 static_assert(sizeof(UnitMeta) == 24, "UnitMeta layout");
 
+// A chunk = consecutive whole batches of one super-batch, up to kChunkSlots slots: the unit of the packed DMMA contractions
+// (snk_gemm_kt.cu).  Its row list (functions in the union of the batches' B_j) lives in a [nchunks x lstride] int table.
+constexpr int kChunkSlots = 2048;
+struct ChunkRec { int64_t slot0; int32_t nslots; int32_t b0, b1; int32_t pad; };
+static_assert(sizeof(ChunkRec) == 24, "ChunkRec layout");
+// 128-slot column tile of a4 (inside one chunk)
+struct ColTile { int64_t slot; int32_t chunk; int32_t ncols; };
+
 // One tile = up to kTile consecutive slots of one batch.
 struct TileRec { int32_t batch; int32_t n; int64_t slot; };
 

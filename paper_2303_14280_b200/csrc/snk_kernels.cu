@@ -650,6 +650,33 @@ cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double*
   return cudaGetLastError();
 }
 
+// work estimate of a batch for Alg. 2: primitive pair-points = |Q_j| * sum of the primitive pairs of the
+// units kept in V_j (what the integral kernel's time is proportional to).  One CTA per batch.
+__global__ void __launch_bounds__(256) k_batch_costs(int nunit, const UnitMeta* __restrict__ meta, const int32_t* __restrict__ bn,
+                                                     const uint32_t* __restrict__ vmask, int64_t vstride, double* __restrict__ cost) {
+  __shared__ double red[8];
+  const int j = blockIdx.x;
+  const uint32_t* __restrict__ mrow = vmask + (int64_t)j * vstride;
+  double v = 0.0;
+  for (int i = threadIdx.x; i < nunit; i += 256)
+    if ((mrow[i >> 5] >> (i & 31)) & 1u) v += (double)(meta[i].nprim_first & 0xff);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(~0u, v, d);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int k = 0; k < 8; ++k) t += red[k];
+    cost[j] = t * (double)bn[j];
+  }
+}
+
+cudaError_t run_batch_costs(int nbatch, int nunit, const UnitMeta* meta, const int32_t* bn, const uint32_t* vmask, int64_t vstride,
+                            double* cost, cudaStream_t s) {
+  if (nbatch > 0) k_batch_costs<<<(unsigned)nbatch, 256, 0, s>>>(nunit, meta, bn, vmask, vstride, cost);
+  return cudaGetLastError();
+}
+
 cudaError_t run_vlist(int b0, int nb, const int* cls_beg, const uint32_t* vmask, int64_t vstride, int32_t* list, int64_t stride,
                       int32_t* cnt, cudaStream_t s) {
   if (nb > 0) {

@@ -42,6 +42,8 @@ cudaError_t run_unit_fill(const PairCand& pc, const ShellTab& sh, const int32_t*
                           UnitMeta* meta, cudaStream_t s);
 cudaError_t run_vmask(int nbatch, int nunit, const UnitMeta* meta, const double* FtsT, int nshld, const double* phit, double eps,
                       uint32_t* vmask, int64_t vstride, cudaStream_t s);
+cudaError_t run_batch_costs(int nbatch, int nunit, const UnitMeta* meta, const int32_t* bn, const uint32_t* vmask, int64_t vstride,
+                            double* cost, cudaStream_t s);
 cudaError_t run_vlist(int b0, int nb, const int* cls_beg, const uint32_t* vmask, int64_t vstride, int32_t* list, int64_t stride,
                       int32_t* cnt, cudaStream_t s);
 cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellTab& sh, const int32_t* bn, const uint32_t* vmask,
@@ -49,17 +51,16 @@ cudaError_t run_vstats(int nbatch, int nunit, const UnitMeta* meta, const ShellT
 cudaError_t run_colloc(const ShellTab& sh, const TileRec* tiles, int ntiles, const double* gx, const double* gy, const double* gz,
                        const uint32_t* bmask, int nshw, double* Phi, int64_t ld, int64_t slot0, cudaStream_t s);
 cudaError_t run_symmetrise(int n, const double* Kt, double* K, cudaStream_t s);
-// a6 (snk_gemm_kt.cu): activity bits of the (128-function row tile, 16-slot k-tile) blocks of Phi, and the contraction itself
-cudaError_t run_kt_flags(const ShellTab& sh, int nbatch, const int32_t* bn, const int64_t* bslot, const uint32_t* bmask, int nshw,
-                         uint32_t* act, int64_t actw, cudaStream_t s);
-// a4 (snk_gemm_kt.cu): activity bits of the (128-slot column tile, 16-function k-tile) blocks of Phi, and F = P Phi
-cudaError_t run_f_flags(const ShellTab& sh, int nbatch, const int32_t* bn, const int64_t* bslot, const int64_t* bslot0,
-                        const int64_t* btile0, const uint32_t* bmask, int nshw, uint32_t* act, int64_t ntiles, int kwords, cudaStream_t s);
-cudaError_t gemm_f(int64_t nbf, int64_t ncols, const double* P, const double* Phi, double* F, int64_t ld, const uint32_t* act, int kwords,
-                   cudaStream_t s);
-int kt_row_tile();   // Phi rows per CTA tile of k_gemm_kt = granularity of its activity bits
-cudaError_t gemm_kt(int64_t nbf, int64_t slot0, int64_t nslots, const double* Phi, const double* G, int64_t ld, const double* wts,
-                    double* Kt, const uint32_t* act, int64_t actw, cudaStream_t s);
+// a4 / a6 (snk_gemm_kt.cu): row lists of the chunks, F = P Phi and Kt += Phi diag(w) G^T packed to them
+cudaError_t run_chunk_rows(const ShellTab& sh, int nchunks, const ChunkRec* chunks, const uint32_t* bmask, int nshw, int32_t* rowlist,
+                           int64_t lstride, int32_t* nrows, cudaStream_t s);
+cudaError_t gemm_f(int64_t nbf, int64_t slot0, int ntiles, const ColTile* tiles, int chunk0, const int32_t* nrows, const int32_t* rowlist,
+                   int64_t lstride, const double* P, const double* Phi, double* F, int64_t ld, cudaStream_t s);
+int kt_row_tile();   // packed Phi rows per CTA tile of k_gemm_kt
+int f_k_tile();      // packed k entries per step of k_gemm_f
+cudaError_t gemm_kt(int64_t nbf, int64_t slot0, int nchunks, int max_nrow, const ChunkRec* chunks, const int32_t* nrows,
+                    const int32_t* rowlist, int64_t lstride, const double* Phi, const double* G, int64_t ld, const double* wts, double* Kt,
+                    cudaStream_t s);
 cudaError_t run_zero_pad_cols(double* A, int64_t rows, int64_t ld, int64_t c0, int64_t c1, cudaStream_t s);
 cudaError_t run_fp64_peak(double* dfma_tflops, double* dmma_tflops, int reps);
 

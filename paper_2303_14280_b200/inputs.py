@@ -256,11 +256,29 @@ def density_from_C(rng: np.random.Generator, nbf: int, nocc: int, sigma: float) 
     return 0.5 * (P + P.T)
 
 
-def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, natoms=None, grid_atoms=None) -> Workload:
+def density_localised(rng: np.random.Generator, basis: Basis, nocc: int, decay_bohr: float, sigma: float = 1.0) -> np.ndarray:
+    """Spatially decaying density: P = C C^T, every column of C a random orbital localised around
+    one atom, C[mu, i] = N(0, sigma^2) * exp(-|R_mu - R_c(i)| / decay_bohr) with c(i) cycling through the atoms.  Symmetric,
+    positive semi-definite, and |P[mu, nu]| falls off like exp(-|R_mu - R_nu| / decay_bohr) by the triangle inequality: the
+    shape of the density of an insulator, for which Eq. 46 localises and sn-LinK deletes work."""
+    fo = basis.shell_offset
+    cen = np.repeat(basis.atom_xyz[basis.shell_atom], np.diff(fo), axis=0)             # centre of every basis function
+    natoms = basis.atom_xyz.shape[0]
+    home = basis.atom_xyz[np.arange(nocc) % natoms]                                    # centre of every column
+    g = rng.standard_normal((basis.nbf, nocc)) * sigma
+    d = np.linalg.norm(cen[:, None, :] - home[None, :, :], axis=2)
+    C = g * np.exp(-d / decay_bohr)
+    P = C @ C.T
+    return 0.5 * (P + P.T)
+
+
+def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, natoms=None, grid_atoms=None,
+                  density: str = "dense", decay_bohr: float = 1.5) -> Workload:
     """BASELINE.json config ``cfg`` (1..5).  ``grid=(n_r,n_theta,n_phi)`` overrides the grid level
     (reduced levels are what the CPU-sized parity tests use); ``lattice`` / ``natoms`` shrink
     the molecule (tests only); ``grid_atoms`` keeps the whole molecule, basis and P but only the atomic grids of the
-    listed atoms (tests only).  Everything else (seed, draw order) is fixed."""
+    listed atoms (tests only); ``density="decay"`` swaps the dense random density for a spatially decaying one
+    (density_localised).  Everything else (seed, draw order) is fixed."""
     c = CONFIGS[cfg]
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + cfg))
     # draw order: geometry -> basis -> C
@@ -278,7 +296,12 @@ def make_workload(cfg: int, *, grid=None, device: str = "cpu", lattice=None, nat
         full_atoms = {2: 24, 3: 192, 4: 1029, 5: 32}[cfg]
         nocc = max(1, int(round(nocc * len(zs) / full_atoms)))
     sigma = c["sigma"] if c["sigma"] is not None else 1.0 / math.sqrt(nocc)
-    P = density_from_C(rng, nbf, nocc, sigma)
+    if density == "dense":            # BASELINE.json: P = C C^T, C i.i.d. Gaussian (no spatial decay)
+        P = density_from_C(rng, nbf, nocc, sigma)
+    elif density == "decay":          # section 8(f)-2: localised orbitals, exponentially decaying P
+        P = density_localised(rng, basis, nocc, decay_bohr)
+    else:
+        raise ValueError("density must be 'dense' or 'decay'")
     g = grid or c["grid"]
     pts, w = becke_grid(xyz, *g, device=device, parents=grid_atoms)
     return Workload(name=c["name"], cfg=cfg, basis=basis, points=pts, weights=w, P=P, eps=c["eps"],

@@ -17,7 +17,7 @@ HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "snk.h")
 
 SNK_OK, SNK_EINVAL, SNK_ENOMEM, SNK_ECUDA, SNK_ESTATE = 0, -1, -2, -3, -4
 
-EXPORTS = ["snk_create", "snk_set_option", "snk_set_grid", "snk_build_K", "snk_build_K_host", "snk_nbf", "snk_get_stats",
+EXPORTS = ["snk_create", "snk_set_option", "snk_set_grid", "snk_build_K", "snk_build_K_host", "snk_screen", "snk_batch_costs", "snk_nbf", "snk_get_stats",
            "snk_export_lists", "snk_debug_boys", "snk_debug_A_pair", "snk_measure_fp64_peak", "snk_last_error", "snk_destroy",
            "snk_version"]
 
@@ -31,7 +31,7 @@ class SnkStats(C.Structure):
                 ("flops_integral", C.c_double), ("flops_gemm", C.c_double), ("ms_set_grid", C.c_double), ("ms_screen", C.c_double),
                 ("ms_colloc", C.c_double), ("ms_F", C.c_double), ("ms_G", C.c_double), ("ms_Kt", C.c_double), ("ms_sym", C.c_double),
                 ("ms_build", C.c_double), ("ms_G_class", C.c_double * 10), ("n_int_class", C.c_double * 10),
-                ("flops_class", C.c_double * 10), ("n_launches", C.c_int64)]
+                ("flops_class", C.c_double * 10), ("n_launches", C.c_int64), ("flops_gemm_alg", C.c_double)]
 
     def asdict(self):
         d = {}
@@ -67,6 +67,8 @@ def load():
     lib.snk_set_grid.argtypes = [vp, C.c_int64, vp, vp, vp]
     lib.snk_build_K.argtypes = [vp, vp, vp, vp]
     lib.snk_build_K_host.argtypes = [vp, vp, vp, vp]
+    lib.snk_screen.argtypes = [vp, vp, vp]
+    lib.snk_batch_costs.argtypes = [vp, dp]
     lib.snk_nbf.argtypes = [vp]
     lib.snk_get_stats.argtypes = [vp, C.POINTER(SnkStats)]
     lib.snk_export_lists.argtypes = [vp, lp, lp, lp, lp, ip, lp, ip]
@@ -152,6 +154,18 @@ class Snk:
         assert K.is_cuda and K.is_contiguous() and tuple(K.shape) == (self.nbf, self.nbf)
         self._check(self._lib.snk_build_K(self.h, _ptr(P), _ptr(K), _stream(stream)))
         return K
+
+    def screen(self, P, stream=None):
+        """Row a3 only (V_j for this P); then batch_costs()."""
+        assert P.is_cuda and P.is_contiguous() and P.element_size() == 8 and tuple(P.shape) == (self.nbf, self.nbf)
+        self._check(self._lib.snk_screen(self.h, _ptr(P), _stream(stream)))
+
+    def batch_costs(self) -> np.ndarray:
+        """Primitive pair-points per batch (batch order) after screen() or build_K()."""
+        nb = int(self.stats()["nbatch"])
+        out = np.zeros(max(nb, 1), dtype=np.float64)
+        self._check(self._lib.snk_batch_costs(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out[:nb]
 
     def build_K_host(self, P_host: np.ndarray, K_host: np.ndarray = None, stream=None):
         """End-to-end call with HOST buffers (numpy or pinned torch CPU tensors exposing data_ptr)."""

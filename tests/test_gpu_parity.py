@@ -29,15 +29,28 @@ def snk_mod(torch_cuda):
     return snk
 
 
-def _check_parity(Kg, Ko, tag="", scale_abs=False):
-    """north_star's bar: max|dK| <= 1e-10 and relative Frobenius error <= 1e-11.  ``scale_abs`` (config 5 at full size
-    only): |K|max is 3.9e3 there, so 1e-10 absolute would be 2.5e-14 relative -- about a hundred ulp of
-    the large elements of a sum over 1.2e6 grid points, below what two fp64 evaluations in different summation orders can
-    agree to; the absolute bound is then taken relative to |K|max (the Frobenius bound stays as stated)."""
+REL_FLOOR = 1e-13
+
+
+def _abs_tol(kmax, npts=0):
+    """DESIGN.md section 6, reading R21.  north_star's max|dK| <= 1e-10 is an absolute bound; it is kept wherever fp64 can meet
+    it, i.e. while 1e-10 >= 1e-13 |K|max.  Every term of K is a product of two collocation values and one A integral, and
+    each of those is only defined to a relative accuracy of a few 1e-15 to 1e-14 in fp64: exp(-z r^2) has condition number
+    z r^2 (up to ~35 where it still matters), so two correctly rounded evaluations whose r^2 differ by one ulp differ by
+    8e-15 relative, and the device Boys function is held to 1e-14 (test_boys_device_vs_mpmath).  Two independent fp64
+    implementations therefore agree to about 2..5e-14 |K| on the large elements, whatever the summation order; the bound
+    used is max(1e-10, 1e-13 |K|max).  It exceeds 1e-10 only for config 5 at full size (|K|max = 5.4e3: 5.4e-10, observed
+    2.5e-10 = 4.7e-14 |K|max; there the oracle with long double sums moves by 3e-12 and two GPU summation orders by 9e-12, so
+    the difference is not summation noise on either side)."""
+    return max(ABS_TOL, REL_FLOOR * float(kmax))
+
+
+def _check_parity(Kg, Ko, tag="", npts=0):
+    """north_star's bar: max|dK| <= 1e-10 and relative Frobenius error <= 1e-11 (``npts``: grid points of the build, for R21)."""
     d = np.abs(Kg - Ko).max()
     fro = np.linalg.norm(Kg - Ko) / max(np.linalg.norm(Ko), 1e-300)
-    tol = ABS_TOL * (max(1.0, np.abs(Ko).max()) if scale_abs else 1.0)
-    assert d <= tol and fro <= FRO_TOL, "%s: max|dK|=%.3e relF=%.3e (|K|max=%.3e)" % (tag, d, fro, np.abs(Ko).max())
+    tol = _abs_tol(np.abs(Ko).max(), npts)
+    assert d <= tol and fro <= FRO_TOL, "%s: max|dK|=%.3e (tol %.3e) relF=%.3e (|K|max=%.3e)" % (tag, d, tol, fro, np.abs(Ko).max())
     return d, fro
 
 
@@ -113,7 +126,7 @@ def _run_both(snk_mod, oracle_mod, w, *, eps=None, batch_max=2048, batch_cell=6.
         st = ctx.stats()
         os_ = o.stats()
         assert st["n_int_contracted"] == os_["n_int_contracted"], (tag, st["n_int_contracted"], os_["n_int_contracted"])
-    d, fro = _check_parity(Kg, Ko, tag)
+    d, fro = _check_parity(Kg, Ko, tag, npts=w.points.shape[0])
     assert np.array_equal(Kg, Kg.T)
     print("%s: max|dK|=%.2e relF=%.2e |K|max=%.2e nbatch=%d" % (tag, d, fro, np.abs(Ko).max(), ctx.stats()["nbatch"]))
     return Kg, Ko, ctx
@@ -212,10 +225,12 @@ def test_K_cfg2_full_size(snk_mod, oracle_mod):
     _run_both(snk_mod, oracle_mod, w, tag="cfg2-full")
 
 
-def _full_size_sampled(snk_mod, oracle_mod, torch, cfg, frac, tag, scale_abs=False):
+def _full_size_sampled(snk_mod, oracle_mod, torch, cfg, frac, tag):
     """K~ is a plain sum over batches and a subset made of whole root cells reproduces the batches of
-    the full grid (R13).  So with S a small whole-root-cell sample:  K(all) = K(S) + K(rest) up to rounding, and K(S) is
-    small enough for the oracle.  Ties the full-size launch to the oracle through a sample of its outputs' addends."""
+    the full grid (R13).  So with S a whole-root-cell sample:  K(all) = K(S) + K(rest) up to rounding, and K(S) is
+    small enough for the oracle (about two minutes of its time).  Ties the full-size launch to the oracle through a sample of
+    its outputs' addends.  The oracle's K(S) is also evaluated with long double sums (same terms, same order), which says
+    how much of the difference is the oracle's own fp64 rounding."""
     from paper_2303_14280_b200.dist import root_cell_sample
     w = inputs.make_workload(cfg, device="cuda")
     m = root_cell_sample(w.points, 6.0, frac)
@@ -235,31 +250,136 @@ def _full_size_sampled(snk_mod, oracle_mod, torch, cfg, frac, tag, scale_abs=Fal
     assert st_all["nbatch"] == st_S["nbatch"] + st_R["nbatch"]
     assert st_all["n_int_contracted"] == st_S["n_int_contracted"] + st_R["n_int_contracted"]
     assert np.array_equal(K_all, K_all.T)
-    _check_parity(K_S + K_R, K_all, tag + " additivity", scale_abs)
+    da, _ = _check_parity(K_S + K_R, K_all, tag + " additivity", npts=len(m))
     o = oracle_mod.Oracle(w.basis)
     o.set_grid(w.points[m], w.weights[m], eps=w.eps)
     Ko = o.build_K(w.P)
     assert o.stats()["n_int_contracted"] == st_S["n_int_contracted"]
-    d, fro = _check_parity(K_S, Ko, tag + " sample vs oracle", scale_abs)
-    print("%s: %d of %d points in the sample, max|dK|=%.2e relF=%.2e" % (tag, int(m.sum()), len(m), d, fro))
+    d, fro = _check_parity(K_S, Ko, tag + " sample vs oracle", npts=int(m.sum()))
+    Kx = o.build_K(w.P, extended=True)
+    dx, frox = _check_parity(K_S, Kx, tag + " sample vs oracle with long double sums", npts=int(m.sum()))
+    print("%s: %d of %d points in the sample (%.2f%%), |K_S|max=%.3e |K|max=%.3e; GPU vs oracle max|dK|=%.2e relF=%.2e; "
+          "GPU vs oracle(long double sums) %.2e / %.2e; oracle fp64 vs long double sums %.2e; additivity (GPU vs GPU, full size) %.2e"
+          % (tag, int(m.sum()), len(m), 100.0 * m.sum() / len(m), np.abs(Ko).max(), np.abs(K_all).max(), d, fro, dx, frox,
+             np.abs(Ko - Kx).max(), da))
 
 
 def test_K_cfg3_full_size_sampled(snk_mod, oracle_mod, torch_cuda):
-    """configs[2] (64 waters, 1600 functions, 3.9M points, eps 1e-11) at full size."""
-    _full_size_sampled(snk_mod, oracle_mod, torch_cuda, 3, 0.004, "cfg3-full")
+    """configs[2] (64 waters, 1600 functions, 3.9M points, eps 1e-11) at full size; 2 % of the grid meets the oracle."""
+    _full_size_sampled(snk_mod, oracle_mod, torch_cuda, 3, 0.02, "cfg3-full")
 
 
 def test_K_cfg5_full_size_sampled(snk_mod, oracle_mod, torch_cuda):
-    """configs[4] (32 atoms with s..f shells, 992 functions, 1.24M points, eps 1e-12) at full size: all ten classes."""
-    _full_size_sampled(snk_mod, oracle_mod, torch_cuda, 5, 0.004, "cfg5-full", scale_abs=True)
+    """configs[4] (32 atoms with s..f shells, 992 functions, 1.24M points, eps 1e-12) at full size: all ten classes;
+    3 % of the grid meets the oracle.  No scaled tolerance: the bound is R21's."""
+    _full_size_sampled(snk_mod, oracle_mod, torch_cuda, 5, 0.03, "cfg5-full")
+
+
+def _cfg4_root_cell_subset(w, max_points):
+    """Whole root cells of config 4's grid in R13 hash order, each taken if it still fits ``max_points`` (deterministic)."""
+    from paper_2303_14280_b200.dist import root_cell_keys
+    key = root_cell_keys(w.points, w.batch_cell)
+    uniq, inv, cnt = np.unique(key, return_inverse=True, return_counts=True)
+    h = (uniq.astype(np.uint64) * np.uint64(0x9E3779B97F4A7C15)) >> np.uint64(11)
+    chosen = np.zeros(len(uniq), dtype=bool)
+    left = max_points
+    for c in np.lexsort((uniq, h)):
+        if cnt[c] <= left:
+            chosen[c] = True
+            left -= int(cnt[c])
+    return chosen[inv]
 
 
 def test_K_cfg4_subgrid(snk_mod, oracle_mod):
-    """configs[3] (343 waters, 8575 functions, eps 1e-10): the whole molecule, basis and density, on a piece of its grid the
-    oracle can afford -- 1500 seeded points out of the atomic grids of one central water (about 3.3e6 contracted integrals per
-    point: every significant pair survives the screening with this density).  Same points to both sides, lists audited."""
-    w = inputs.make_workload(4, grid_atoms=[513, 514, 515], device="cuda")
-    rng = np.random.Generator(np.random.PCG64(inputs.SEED_BASE + 44))
-    sel = np.sort(rng.choice(w.points.shape[0], size=1500, replace=False))
-    w.points, w.weights = np.ascontiguousarray(w.points[sel]), np.ascontiguousarray(w.weights[sel])
-    _run_both(snk_mod, oracle_mod, w, batch_max=256, tag="cfg4-subgrid")
+    """configs[3] (343 waters, 8575 functions, eps 1e-10): the whole molecule, basis and density on WHOLE ROOT CELLS of its
+    full grid (R13: the same batches as in the full build), default batching (N_max 2048), as many cells as the oracle does
+    in about three minutes (3.3e6 contracted integrals per point: every significant pair survives the screening with this
+    density).  Same points to both sides, lists audited.  The 1 % subset of BASELINE.json is test_K_cfg4_one_percent."""
+    w = inputs.make_workload(4, device="cuda")
+    m = _cfg4_root_cell_subset(w, 6000)
+    assert m.sum() > 3000
+    w.points, w.weights = np.ascontiguousarray(w.points[m]), np.ascontiguousarray(w.weights[m])
+    _run_both(snk_mod, oracle_mod, w, tag="cfg4-rootcells")
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("SNK_RUN_SLOW"), reason="about 1.5 h of oracle time: set SNK_RUN_SLOW=1")
+def test_K_cfg4_one_percent(snk_mod, oracle_mod):
+    """BASELINE.json configs[3]: "the oracle is run only on a deterministic 1 % subset of grid batches" -- whole root cells in
+    R13 hash order until 1 % of the points (R13: that is 1 % of the batches of the full build, unchanged), default batching.
+    The log of the last run is kept under profiles/."""
+    from paper_2303_14280_b200.dist import root_cell_sample
+    w = inputs.make_workload(4, device="cuda")
+    m = root_cell_sample(w.points, w.batch_cell, 0.01)
+    w.points, w.weights = np.ascontiguousarray(w.points[m]), np.ascontiguousarray(w.weights[m])
+    _run_both(snk_mod, oracle_mod, w, tag="cfg4-1pct (%d points)" % int(m.sum()))
+
+
+def test_two_contexts_on_a_side_stream(snk_mod, oracle_mod, torch_cuda):
+    """Two live contexts built on a non-default stream, interleaved: each K equals its oracle K."""
+    torch = torch_cuda
+    wa = inputs.make_workload(2, grid=(10, 6, 12), lattice=1)
+    wb = inputs.make_workload(5, grid=(8, 6, 8), natoms=3)
+    st = torch.cuda.Stream()
+    res = []
+    with torch.cuda.stream(st):
+        ctxs = []
+        for w in (wa, wb):
+            s = snk_mod.Snk(w.basis)
+            s.set_option("eps", w.eps)
+            s.set_grid(torch.as_tensor(w.points, device="cuda"), torch.as_tensor(w.weights, device="cuda"), stream=st)
+            ctxs.append(s)
+        Ps = [torch.as_tensor(w.P, device="cuda") for w in (wa, wb)]
+        for rep in range(2):                      # interleaved builds on the side stream
+            res = [s.build_K(P, stream=st) for s, P in zip(ctxs, Ps)]
+    st.synchronize()
+    for w, K in zip((wa, wb), res):
+        o = oracle_mod.Oracle(w.basis)
+        o.set_grid(w.points, w.weights, eps=w.eps)
+        _check_parity(K.cpu().numpy(), o.build_K(w.P), "two contexts, side stream", npts=w.points.shape[0])
+
+
+def test_sharded_build_on_one_gpu(snk_mod, oracle_mod, torch_cuda):
+    """SURVEY.md section 8(f)-1 / Alg. 1-2 on ONE device: root cells dealt to 3 shards by greedy LPT on the
+    primitive pair-point costs of a screening pass (snk_screen + snk_batch_costs), every shard built through the C ABI, the
+    partial K summed (what the all-reduce of Alg. 1 line 13 does) and compared with the oracle's UNSHARDED K.  The shards'
+    batches are exactly the oracle's batches, their integral counts add up to the oracle's."""
+    from paper_2303_14280_b200 import dist
+    torch = torch_cuda
+    w = inputs.make_workload(2, grid=(16, 8, 14))
+    world = 3
+    o = oracle_mod.Oracle(w.basis)
+    o.set_grid(w.points, w.weights, eps=w.eps, batch_max=512)
+    Ko = o.build_K(w.P)
+    ooff, operm, _ = o.batches()
+    oracle_batches = {frozenset(operm[ooff[j]:ooff[j + 1]].tolist()) for j in range(len(ooff) - 1)}
+    P = torch.as_tensor(w.P, device="cuda")
+    s = snk_mod.Snk(w.basis)
+    s.set_option("eps", w.eps); s.set_option("batch_max", 512)
+    s.set_grid(torch.as_tensor(w.points, device="cuda"), torch.as_tensor(w.weights, device="cuda"))
+    s.screen(P)
+    costs = s.batch_costs()
+    L = s.export_lists(want_V=False)
+    assert costs.shape[0] == len(L["batch_off"]) - 1 and costs.min() >= 0 and costs.sum() > 0
+    cells = dist.root_cell_costs(w.points, w.batch_cell, L["batch_off"], L["perm"], costs)
+    assert abs(cells[1].sum() - costs.sum()) <= 1e-9 * costs.sum()
+    masks = [dist.shard_points(w.points, w.batch_cell, r, world, cell_costs=cells) for r in range(world)]
+    assert np.array_equal(np.sum(masks, axis=0), np.ones(len(w.points)))           # a partition of the grid
+    Ksum = np.zeros_like(Ko)
+    seen, n_int, loads = set(), 0.0, []
+    for m in masks:
+        idx = np.nonzero(m)[0]
+        s.set_grid(torch.as_tensor(np.ascontiguousarray(w.points[idx]), device="cuda"),
+                   torch.as_tensor(np.ascontiguousarray(w.weights[idx]), device="cuda"))
+        Ksum += s.build_K(P).cpu().numpy()
+        Ls = s.export_lists(want_V=False)
+        for j in range(len(Ls["batch_off"]) - 1):
+            seen.add(frozenset(idx[Ls["perm"][Ls["batch_off"][j]:Ls["batch_off"][j + 1]]].tolist()))
+        n_int += s.stats()["n_int_contracted"]
+        loads.append(s.batch_costs().sum())
+    assert seen == oracle_batches
+    assert n_int == o.stats()["n_int_contracted"]
+    _check_parity(Ksum, Ko, "3 shards on one GPU", npts=len(w.points))
+    # costs are additive over root cells up to the primitive screening R14, whose threshold uses maxima over the grid handed in
+    assert abs(sum(loads) - costs.sum()) <= 0.01 * costs.sum()
+    assert max(loads) <= 1.5 * np.mean(loads), loads                                # LPT balance on the work model
+    print("shard loads (primitive pair-points):", ["%.3g" % x for x in loads])
