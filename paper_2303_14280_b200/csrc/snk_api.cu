@@ -937,11 +937,12 @@ int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double
     for (int l = 0; l < ctx->h_nprim[sb]; ++l) {
       const double za = ctx->h_pexp[ctx->h_poff[sa] + k], zb = ctx->h_pexp[ctx->h_poff[sb] + l];
       PrimPair q;
-      q.p = za + zb; q.inv2p = 0.5 / q.p;
-      q.Px = (za * A[0] + zb * B[0]) / q.p; q.Py = (za * A[1] + zb * B[1]) / q.p; q.Pz = (za * A[2] + zb * B[2]) / q.p;
+      const double ps = za + zb;
+      q.p2 = 2.0 * ps; q.inv2p = 0.5 / ps;
+      q.Px = (za * A[0] + zb * B[0]) / ps; q.Py = (za * A[1] + zb * B[1]) / ps; q.Pz = (za * A[2] + zb * B[2]) / ps;
       q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
-      q.pref = ctx->h_pcoef[ctx->h_poff[sa] + k] * ctx->h_pcoef[ctx->h_poff[sb] + l] * (2.0 * M_PI / q.p) * std::exp(-(za * zb / q.p) * AB2);
-      q.cfar = 0.88622692545275801365 * q.pref;
+      q.pref = ctx->h_pcoef[ctx->h_poff[sa] + k] * ctx->h_pcoef[ctx->h_poff[sb] + l] * (2.0 * M_PI / ps) * std::exp(-(za * zb / ps) * AB2);
+      q.cfar2 = 1.2533141373155002512 * q.pref;
       pp.push_back(q);
     }
   DevBuf<PrimPair> d;

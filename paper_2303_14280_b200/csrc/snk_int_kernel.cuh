@@ -6,10 +6,12 @@
 //   * the V_j bit masks are expanded once per super-batch into per-(batch, class) unit-id lists (k_vlist); the warps of a tile
 //     that cover the same points (a point group: 4 of the 8 warps for L <= 1, 2 for L = 2) take the list's entries round robin;
 //   * every warp streams ITS units -- header + primitive pairs (<= 704 B) and the F_b row segments of its points -- through a
-//     private ring of D shared-memory slots with cp.async.bulk (TMA bulk copy) completing on a per-slot mbarrier: lane 0 refills
-//     a slot as soon as the warp has finished the unit in it, D units ahead, so the recurrences run against broadcast LDS only
-//     and never wait for global memory.  No producer warp (a ninth warp costs every thread of the CTA a quarter of its registers:
-//     CTAs are allocated in warp pairs), no tickets, no barrier shared between warps;
+//     private ring of D shared-memory slots with 16-byte cp.async copies, one commit group per unit: the warp refills a slot as
+//     soon as it has finished the unit in it, D units ahead, so the recurrences run against broadcast LDS only and never wait
+//     for global memory.  No producer warp (a ninth warp costs every thread of the CTA a quarter of its registers: CTAs are
+//     allocated in warp pairs), no tickets, no barrier shared between warps.  (Bulk copies completing on mbarriers were
+//     measured first: one elected lane pays ~60 instructions per unit for the uniform-register set-up of 1 + ncart(l_b) copies;
+//     the per-lane 16-byte copies cost a fifth of that and need no barrier objects.);
 //   * a thread owns NP points of the tile (2 for L <= 1, else 1): the point-independent work of a unit is paid once per 32 NP
 //     points and the NP recurrences are independent instruction streams;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
@@ -31,7 +33,7 @@ namespace snk {
 #define SNK_NP_L0 4
 #endif
 #ifndef SNK_NP_L1
-#define SNK_NP_L1 4
+#define SNK_NP_L1 2
 #endif
 #ifndef SNK_NP_L2
 #define SNK_NP_L2 2
@@ -48,7 +50,7 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
 #define SNK_MB_L0 2
 #endif
 #ifndef SNK_MB_L1
-#define SNK_MB_L1 3
+#define SNK_MB_L1 2
 #endif
 #ifndef SNK_MB_L2
 #define SNK_MB_L2 3
@@ -69,7 +71,7 @@ __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
 #define SNK_CW_L0 8
 #endif
 #ifndef SNK_CW_L1
-#define SNK_CW_L1 4
+#define SNK_CW_L1 8
 #endif
 #ifndef SNK_CW_L2
 #define SNK_CW_L2 4
@@ -92,6 +94,12 @@ __host__ __device__ constexpr int int_cw(int LA, int LB) {
 }
 __host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_cw(LA, LB); }
 
+// F_a of the current a-run: held in registers (0) or re-read through L1 when the unit's recurrences are done (1); the second
+// takes ncart(l_a) NP doubles off the register budget of the primitive loop
+#ifndef SNK_FA_RELOAD_L1
+#define SNK_FA_RELOAD_L1 0
+#endif
+__host__ __device__ constexpr bool int_fa_reload(int LA, int LB) { return LA + LB == 1 && SNK_FA_RELOAD_L1 != 0; }
 // depth of a warp's prefetch ring (a power of two): units in flight ahead of the one being evaluated
 #ifndef SNK_D_L0
 #define SNK_D_L0 8
@@ -108,87 +116,28 @@ __host__ __device__ constexpr int int_threads(int LA, int LB) { return 32 * int_
 __host__ __device__ constexpr int int_depth(int LA, int LB) { return LA + LB == 0 ? SNK_D_L0 : LA + LB == 1 ? SNK_D_L1 : LA + LB == 2 ? SNK_D_L2 : SNK_D_LHI; }
 // one ring slot of a warp: the unit record, then ncart(l_b) row segments of F for the 32 NP points of the warp
 __host__ __device__ constexpr int int_slot_bytes(int LB, int NP) { return kUnitBytes + ncart(LB) * 32 * NP * 8; }
-// per warp: D slots; then D full-mbarriers per warp
-__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) {
-  return int_cw(LA, LB) * int_depth(LA, LB) * (int_slot_bytes(LB, int_npmax(LA, LB)) + 8);
-}
+// per warp: D slots
+__host__ __device__ constexpr int int_smem_bytes(int LA, int LB) { return int_cw(LA, LB) * int_depth(LA, LB) * int_slot_bytes(LB, int_npmax(LA, LB)); }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+__device__ __forceinline__ void cp16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "SNK_WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra SNK_DONE_%=;\n"
-      "bra SNK_WAIT_%=;\n"
-      "SNK_DONE_%=:\n"
-      "}\n" ::"r"(bar),
-      "r"(parity)
-      : "memory");
-}
-// producer-side wait: try_wait suspends the lane in hardware until the phase completes or the time hint (ns) expires, so the
-// waiting producer takes (almost) no issue slots from the consumer warps
-__device__ __forceinline__ void mbar_wait_suspend(uint32_t bar, uint32_t parity) {
-  uint32_t done;
-  do {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n"
-        : "=r"(done)
-        : "r"(bar), "r"(parity), "r"(1000000u)
-        : "memory");
-  } while (!done);
-}
-// non-blocking probe (the consumer issues it one unit ahead, so the barrier round trip overlaps the recurrences)
-__device__ __forceinline__ uint32_t mbar_test(uint32_t bar, uint32_t parity) {
-  uint32_t done;
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-      "selp.u32 %0, 1, 0, p;\n"
-      "}\n"
-      : "=r"(done)
-      : "r"(bar), "r"(parity)
-      : "memory");
-  return done;
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
-               "r"(bar)
-               : "memory");
-}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- one warp: its share (entries rnk, rnk + WPG, ... of the list) of the tile's unit stream for the points
 // [pbase, pbase + 32 NP) of the tile, NP per thread ----
 template <int LA, int LB, int NP, int WPG>
 __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec& tile, const int32_t* __restrict__ list, int cnt,
-                                              unsigned char* ring, uint32_t s_bar, int pbase, int rnk, int lane) {
+                                              unsigned char* ring, int pbase, int rnk, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
   constexpr int D = int_depth(LA, LB), SLOT = int_slot_bytes(LB, int_npmax(LA, LB));
   constexpr uint32_t FROW = 32u * NP * 8u;             // bytes of one staged F row segment
   const int n_my = cnt > rnk ? (cnt - rnk + WPG - 1) / WPG : 0;
   if (n_my == 0) return;
   const uint32_t s_ring = smem_u32(ring);
-  if (lane == 0) {
-#pragma unroll
-    for (int i = 0; i < D; ++i) mbar_init(s_bar + 8 * i, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncwarp();
 
   int pt[NP], ptc[NP];
   bool act[NP];
@@ -216,24 +165,30 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
       m = mm.x | (mm.y & 0xff) << 24;
     }
   };
-  // stage this warp's k-th unit into slot k % D
+  // stage this warp's k-th unit into slot k % D: 16-byte chunks, lane by lane (a unit record is at most 44 chunks, a row
+  // segment of F 16 NP); k >= n_my only closes an (empty) commit group, which keeps "group k = unit k"
   auto issue = [&](int k, int e_w, int m_w) {
-    const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
-    if (lane == 0) {
-      const uint32_t slot = (uint32_t)k % D, bar = s_bar + 8 * slot, dst = s_ring + slot * SLOT;
-      const uint32_t nb = 64u + ((uint32_t)m >> 24) * (uint32_t)kPrimBytes;
-      // (the slot was only READ through the generic proxy, and every lane's reads precede the __syncwarp: no proxy fence needed)
-      mbar_arrive_expect_tx(bar, nb + NB * FROW);
-      bulk_g2s(dst, p.units + (size_t)e * kUnitBytes, nb, bar);
-      const double* __restrict__ Fsrc = Fc + (int64_t)(m & 0xffffff) * ld + pbase;
+    if (k < n_my) {
+      const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
+      const uint32_t dst = s_ring + ((uint32_t)k % D) * SLOT + lane * 16;
+      const int nb = 64 + (int)((uint32_t)m >> 24) * kPrimBytes;
+      const unsigned char* __restrict__ src = p.units + (size_t)e * kUnitBytes + lane * 16;
+      if (lane * 16 < nb) cp16(dst, src);
+      if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
+      const double* __restrict__ Fsrc = Fc + (int64_t)(m & 0xffffff) * ld + pbase + lane * 2;
 #pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2) bulk_g2s(dst + kUnitBytes + k2 * FROW, Fsrc + (int64_t)k2 * ld, FROW, bar);
+      for (int k2 = 0; k2 < NB; ++k2)
+#pragma unroll
+        for (int c = 0; c < NP * 16; c += 32)
+          if (c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (int64_t)k2 * ld + c * 2);
     }
+    cp_commit();
   };
   int e0, m0, e1, m1;
   load_win(0, e0, m0);
   load_win(32, e1, m1);
-  for (int k = 0; k < D && k < n_my; ++k) issue(k, e0, m0);
+#pragma unroll
+  for (int k = 0; k < D; ++k) issue(k, e0, m0);
 
   int cur_fa = -1;
   int64_t cur_offa = 0;
@@ -254,9 +209,9 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
 
 #pragma unroll 1
   for (int k = 0; k < n_my; ++k) {
-    const uint32_t sl = (uint32_t)k % D, phase = ((uint32_t)k / D) & 1u;
-    if (!mbar_test(s_bar + 8 * sl, phase)) mbar_wait(s_bar + 8 * sl, phase);
-    const unsigned char* rec = ring + sl * SLOT;
+    cp_wait<D - 1>();                                              // this thread's copies of unit k have landed ...
+    __syncwarp();                                                  // ... and so have those of the other lanes
+    const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
     const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
     const int fa = h0.x, fb = h0.y;
     double ABx = 0.0, ABy = 0.0, ABz = 0.0;
@@ -271,7 +226,10 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) { Fa[s][i] = Fc[off.x + (int64_t)i * ld + ptc[s]]; Ga[s][i] = 0.0; }
+        for (int i = 0; i < NA; ++i) {
+          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = Fc[off.x + (int64_t)i * ld + ptc[s]];
+          Ga[s][i] = 0.0;
+        }
     }
     double Fb[NP][NB], Gb[NP][NB];
     const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
@@ -282,6 +240,12 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
 
     double acc[NP][nlev(LA, L)];
     theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
+    if constexpr (int_fa_reload(LA, LB)) {
+#pragma unroll
+      for (int s = 0; s < NP; ++s)
+#pragma unroll
+        for (int i = 0; i < NA; ++i) Fa[s][i] = __ldg(Fc + cur_offa + (int64_t)i * ld + ptc[s]);
+    }
 #pragma unroll
     for (int s = 0; s < NP; ++s) {
       ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
@@ -290,10 +254,8 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
 
     __syncwarp();                                                  // every lane is done with the slot: refill it D units ahead
     const int kn = k + D;
-    if (kn < n_my) {
-      if ((kn & 31) == 0) { e0 = e1; m0 = m1; load_win(kn + 32, e1, m1); }
-      issue(kn, e0, m0);
-    }
+    if ((kn & 31) == 0 && kn < n_my) { e0 = e1; m0 = m1; load_win(kn + 32, e1, m1); }
+    issue(kn, e0, m0);
     if (fa != fb) {                                                // a == b (same shell): one direction only
 #pragma unroll
       for (int s = 0; s < NP; ++s)
@@ -325,18 +287,17 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   if (pbase >= tile.n) return;
   const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg;
   unsigned char* ring = smem_int + warp * (D * SLOT);
-  const uint32_t s_bar = smem_u32(smem_int + CW * D * SLOT) + warp * (D * 8);
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
   if constexpr (NPM == 4) {
-    if (need == 4) consume_units<LA, LB, 4, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
-    else if (need == 3) consume_units<LA, LB, 3, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
-    else if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    if (need == 4) consume_units<LA, LB, 4, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else if (need == 3) consume_units<LA, LB, 3, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
   } else if constexpr (NPM == 2) {
-    if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
   } else {
-    consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, s_bar, pbase, rnk, lane);
+    consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
   }
 }
 

@@ -350,12 +350,13 @@ __global__ void k_unit_fill(PairCand pc, ShellTab sh, const int32_t* __restrict_
         if (cca * ccb * (6.283185307179586 / pp) * exp(-(zza * zzb / pp) * AB2) * dens < thr) continue;
       }
       PrimPair q;
-      q.p = za + zb;
-      q.inv2p = 0.5 / q.p;
-      q.Px = (za * A[0] + zb * B[0]) / q.p; q.Py = (za * A[1] + zb * B[1]) / q.p; q.Pz = (za * A[2] + zb * B[2]) / q.p;
+      const double pp = za + zb;
+      q.p2 = 2.0 * pp;
+      q.inv2p = 0.5 / pp;
+      q.Px = (za * A[0] + zb * B[0]) / pp; q.Py = (za * A[1] + zb * B[1]) / pp; q.Pz = (za * A[2] + zb * B[2]) / pp;
       q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
-      q.pref = ca * cb * (6.283185307179586 / q.p) * exp(-(za * zb / q.p) * AB2);
-      q.cfar = 0.88622692545275801365 * q.pref;   // pref sqrt(pi)/2: far-field seed constant
+      q.pref = ca * cb * (6.283185307179586 / pp) * exp(-(za * zb / pp) * AB2);
+      q.cfar2 = 1.2533141373155002512 * q.pref;   // pref sqrt(pi/2): far-field seed constant (snk_os.cuh)
       *reinterpret_cast<PrimPair*>(units + (size_t)(u0 + n / kUnitPrims) * kUnitBytes + 64 + (n % kUnitPrims) * kPrimBytes) = q;
       ++n;
     }

@@ -114,18 +114,27 @@ __device__ __forceinline__ void boys_near(double x, const double* __restrict__ t
   }
 }
 
-// Seeds (A3, R1) Theta^n_0 = pref F_n(x), n = 0..L, with the prefactor folded into the Boys evaluation:
-// far field: Theta^0_0 = cfar / sqrt(x), cfar = pref sqrt(pi)/2, and Theta^{m+1}_0 = Theta^m_0 (2m+1)/(2x): the factors
-// (2m+1) h are formed off the critical path; near field: pref scales F_L and e^{-x} once, the downward recursion is linear.
+// Seeds (A3, R1) Theta^n_0 = pref F_n(x), n = 0..L, with the prefactor folded into the Boys evaluation.  The kernel carries
+// x2 = 2x.  Far field: with r = 1/sqrt(x2), Theta^0_0 = cfar2 r (cfar2 = pref sqrt(pi/2)), 1/(2x) = r r, and
+// Theta^{m+1}_0 = Theta^m_0 (2m+1)/(2x): the factors (2m+1) h are formed off the critical path; near field: pref scales F_L and
+// e^{-x} once, the downward recursion is linear.
+__host__ __device__ constexpr int boys_x2max_hi(int L) {       // high word of the double 2 xmax(L) (its low word is zero)
+  const double v = 2.0 * boys_xmax(L);                         // 68, 76, 80, 88, 92, 100, 104: exact, exponent 6
+  return (int)(0x40500000u + (unsigned)((v - 64.0) * 16384.0));  // 1.f * 2^6: mantissa bits (v/64 - 1) * 2^20
+}
+// x2 >= 2 xmax(L) for a non-negative finite double: an integer compare of the high words (the FP64 pipe is the scarce one)
 template <int L>
-__device__ __forceinline__ void seeds_far(double x, double cfar, double (&T)[L + 1]) {
+__device__ __forceinline__ bool is_far(double x2) { return __double2hiint(x2) >= boys_x2max_hi(L); }
+
+template <int L>
+__device__ __forceinline__ void seeds_far(double x2, double cfar2, double (&T)[L + 1]) {
   double y0;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-  const double e = fma(-x, y0 * y0, 1.0);
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x2));
+  const double e = fma(-x2, y0 * y0, 1.0);
   const double r = fma(fma(e, 0.375, 0.5), y0 * e, y0);
-  T[0] = cfar * r;
+  T[0] = cfar2 * r;
   if constexpr (L > 0) {
-    const double h = (0.5 * r) * r;                // 1/(2x)
+    const double h = r * r;                        // 1/(2x)
     T[1] = T[0] * h;
 #pragma unroll
     for (int m = 1; m < L; ++m) T[m + 1] = T[m] * ((2 * m + 1) * h);
@@ -135,14 +144,14 @@ __device__ __forceinline__ void seeds_far(double x, double cfar, double (&T)[L +
 // warp issues in order, so consecutive instructions must belong to different dependency chains to cover the 8-cycle FP64
 // latency (a Newton step per point in sequence would stall on every instruction).
 template <int L, int N>
-__device__ __forceinline__ void seeds_far_v(const double (&x)[N], const double (&cfar)[N], double (&T)[N][L + 1]) {
+__device__ __forceinline__ void seeds_far_v(const double (&x2)[N], const double (&cfar2)[N], double (&T)[N][L + 1]) {
   double y0[N], e[N], u[N], r[N];
 #pragma unroll
-  for (int i = 0; i < N; ++i) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0[i]) : "d"(x[i]));
+  for (int i = 0; i < N; ++i) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0[i]) : "d"(x2[i]));
 #pragma unroll
   for (int i = 0; i < N; ++i) u[i] = y0[i] * y0[i];
 #pragma unroll
-  for (int i = 0; i < N; ++i) e[i] = fma(-x[i], u[i], 1.0);
+  for (int i = 0; i < N; ++i) e[i] = fma(-x2[i], u[i], 1.0);
 #pragma unroll
   for (int i = 0; i < N; ++i) u[i] = y0[i] * e[i];
 #pragma unroll
@@ -150,13 +159,11 @@ __device__ __forceinline__ void seeds_far_v(const double (&x)[N], const double (
 #pragma unroll
   for (int i = 0; i < N; ++i) r[i] = fma(e[i], u[i], y0[i]);
 #pragma unroll
-  for (int i = 0; i < N; ++i) T[i][0] = cfar[i] * r[i];
+  for (int i = 0; i < N; ++i) T[i][0] = cfar2[i] * r[i];
   if constexpr (L > 0) {
     double h[N];
 #pragma unroll
-    for (int i = 0; i < N; ++i) h[i] = 0.5 * r[i];
-#pragma unroll
-    for (int i = 0; i < N; ++i) h[i] = h[i] * r[i];            // 1/(2x)
+    for (int i = 0; i < N; ++i) h[i] = r[i] * r[i];            // 1/(2x)
 #pragma unroll
     for (int i = 0; i < N; ++i) T[i][1] = T[i][0] * h[i];
 #pragma unroll
@@ -199,9 +206,9 @@ __device__ __forceinline__ void seeds_near(double x, double pref, const double* 
   }
 }
 template <int L>
-__device__ __forceinline__ void seeds(double x, double pref, double cfar, const double* __restrict__ tab, double (&T)[L + 1]) {
-  if (x < boys_xmax(L)) seeds_near<L>(x, pref, tab, T);
-  else seeds_far<L>(x, cfar, T);
+__device__ __forceinline__ void seeds(double x2, double pref, double cfar2, const double* __restrict__ tab, double (&T)[L + 1]) {
+  if (!is_far<L>(x2)) seeds_near<L>(0.5 * x2, pref, tab, T);
+  else seeds_far<L>(x2, cfar2, T);
 }
 
 // per-lane dispatch (test hooks, divergent warps)
@@ -215,12 +222,12 @@ __device__ __forceinline__ void boys(double x, const double* __restrict__ tab, d
 // One primitive pair: everything that does not depend on the grid point.
 // ------------------------------------------------------------------------------------------------
 struct __align__(16) PrimPair {
-  double p;        // zeta_a + zeta_b
+  double p2;       // 2 (zeta_a + zeta_b): the kernel works with 2x = p2 |P - r_g|^2, whose inverse square root gives 1/(2x) in one multiply
   double inv2p;    // 1 / (2p)
   double Px, Py, Pz;
   double PAx, PAy, PAz;   // P - A, A = centre of the shell that carries the VRR (first of the pair, l_a >= l_b)
   double pref;     // c_a c_b (2 pi / p) exp(-zeta_a zeta_b / p |A-B|^2)
-  double cfar;     // pref * sqrt(pi)/2: Theta^0_0 = cfar / sqrt(x) in the far field
+  double cfar2;    // pref * sqrt(pi/2): Theta^0_0 = cfar2 / sqrt(2x) in the far field
 };
 static_assert(sizeof(PrimPair) == 80, "PrimPair layout");
 
@@ -377,7 +384,7 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
 #pragma unroll
     for (int j = 0; j < K; ++j) {
       const double2* __restrict__ q = reinterpret_cast<const double2*>(pp + k + j);
-      q0[j] = q[0]; q1[j] = q[1]; q2[j] = q[2];     // (p, inv2p) (Px, Py) (Pz, PAx)
+      q0[j] = q[0]; q1[j] = q[1]; q2[j] = q[2];     // (p2, inv2p) (Px, Py) (Pz, PAx)
     }
 #pragma unroll
     for (int j = 0; j < K; ++j)
@@ -391,12 +398,12 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
     for (int i = 0; i < N; ++i) x[i] = fma(PCx[i], PCx[i], x[i]);
 #pragma unroll
     for (int i = 0; i < N; ++i) x[i] *= q0[i / NP].x;
-    bool far = true;
+    bool far = true;                                  // x[] holds 2x (p2 = 2p)
 #pragma unroll
-    for (int i = 0; i < N; ++i) far = far && x[i] >= boys_xmax(L);
+    for (int i = 0; i < N; ++i) far = far && is_far<L>(x[i]);
     bool allfar = false;
     if constexpr (WARP) allfar = __all_sync(0xffffffffu, far);
-    double2 q4[K];                                    // (pref, cfar)
+    double2 q4[K];                                    // (pref, cfar2)
 #pragma unroll
     for (int j = 0; j < K; ++j) q4[j] = reinterpret_cast<const double2*>(pp + k + j)[4];
     if (allfar) {
@@ -405,8 +412,14 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
       for (int i = 0; i < N; ++i) cf[i] = q4[i / NP].y;
       seeds_far_v<L, N>(x, cf, th0);
     } else {
+      // chain by chain: a chain whose 32 points are all far still runs without branches or table loads
 #pragma unroll
-      for (int i = 0; i < N; ++i) seeds<L>(x[i], q4[i / NP].x, q4[i / NP].y, boys_tab, th0[i]);
+      for (int i = 0; i < N; ++i) {
+        bool cf = is_far<L>(x[i]);
+        if constexpr (WARP) cf = __all_sync(0xffffffffu, cf);
+        if (cf) seeds_far<L>(x[i], q4[i / NP].y, th0[i]);
+        else seeds<L>(x[i], q4[i / NP].x, q4[i / NP].y, boys_tab, th0[i]);
+      }
     }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
