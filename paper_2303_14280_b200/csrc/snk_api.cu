@@ -526,6 +526,7 @@ int snk_set_grid(snk_ctx* ctx, int64_t npts, const double* points, const double*
           ctx->h_tiles.push_back(TileRec{j, std::min(kTile, ctx->h_bn[j] - o), ctx->h_bslot[j] + o});
       const double budget = ctx->workspace_gb * 1073741824.0;
       int64_t max_slots = (int64_t)(budget / (3.0 * 8.0 * std::max(1, ctx->nbf)));
+      max_slots = std::min<int64_t>(max_slots, (int64_t)500000000);           // the kernels address slab rows with a 32-bit byte stride
       max_slots = std::max<int64_t>(max_slots / 128 * 128, 4096 + kSlotAlign);
       int t = 0;
       for (int j = 0; j < nb;) {

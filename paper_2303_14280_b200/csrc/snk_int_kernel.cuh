@@ -129,7 +129,10 @@ __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0
 
 // ---- one warp: its share (entries rnk, rnk + WPG, ... of the list) of the tile's unit stream for the points
 // [pbase, pbase + 32 NP) of the tile, NP per thread ----
-template <int LA, int LB, int NP, int WPG>
+// FULL: every lane of the warp owns NP points of the tile (no predicates, no clamped indices); ragged groups take FULL = false.
+// Row addresses in the F / G slabs are base + row * ld8 with a 32-bit byte stride ld8 (the host keeps ld * 8 < 2^32): one
+// 32 x 32 -> 64 bit multiply-add per address.
+template <int LA, int LB, int NP, int WPG, bool FULL>
 __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec& tile, const int32_t* __restrict__ list, int cnt,
                                               unsigned char* ring, int pbase, int rnk, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
@@ -139,21 +142,24 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
   if (n_my == 0) return;
   const uint32_t s_ring = smem_u32(ring);
 
-  int pt[NP], ptc[NP];
+  uint32_t pb[NP];                                     // byte offset of this thread's points inside a slab row of the tile
   bool act[NP];
   double gx[NP], gy[NP], gz[NP];
 #pragma unroll
   for (int s = 0; s < NP; ++s) {
-    pt[s] = pbase + 32 * s + lane;
-    act[s] = pt[s] < tile.n;
-    ptc[s] = act[s] ? pt[s] : tile.n - 1;             // inactive lanes shadow the tile's last point and never write
-    const int64_t slot = tile.slot + ptc[s];
+    const int pt = pbase + 32 * s + lane;
+    act[s] = FULL || pt < tile.n;
+    const int ptc = act[s] ? pt : tile.n - 1;         // inactive lanes shadow the tile's last point and never write
+    pb[s] = (uint32_t)ptc * 8u;
+    const int64_t slot = tile.slot + ptc;
     gx[s] = p.gx[slot]; gy[s] = p.gy[slot]; gz[s] = p.gz[slot];
   }
   const int64_t col0 = tile.slot - p.slot0;
-  const double* __restrict__ Fc = p.F + col0;
-  double* __restrict__ Gc = p.G + col0;
-  const int64_t ld = p.ld;
+  const uint32_t ld8 = (uint32_t)p.ld * 8u;
+  const char* __restrict__ Fl = reinterpret_cast<const char*>(p.F + col0);
+  char* __restrict__ Gl = reinterpret_cast<char*>(p.G + col0);
+  auto F_at = [&](int row, int s) { return *reinterpret_cast<const double*>(Fl + (uint64_t)(uint32_t)row * ld8 + pb[s]); };
+  auto G_add = [&](int row, int s, double v) { atomicAdd(reinterpret_cast<double*>(Gl + (uint64_t)(uint32_t)row * ld8 + pb[s]), v); };
 
   // unit ids and (fb | nprim << 24) of this warp's units [32 w, 32 w + 32): lane i holds unit 32 w + i; two windows in flight
   auto load_win = [&](int wb, int& e, int& m) {
@@ -167,20 +173,23 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
   };
   // stage this warp's k-th unit into slot k % D: 16-byte chunks, lane by lane (a unit record is at most 44 chunks, a row
   // segment of F 16 NP); k >= n_my only closes an (empty) commit group, which keeps "group k = unit k"
+  const unsigned char* __restrict__ Ucp = p.units + lane * 16;
+  const char* __restrict__ Fcp = Fl + (pbase * 8 + lane * 16);
+  const uint32_t dst_lane = s_ring + lane * 16;
   auto issue = [&](int k, int e_w, int m_w) {
     if (k < n_my) {
       const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
-      const uint32_t dst = s_ring + ((uint32_t)k % D) * SLOT + lane * 16;
+      const uint32_t dst = dst_lane + ((uint32_t)k % D) * SLOT;
       const int nb = 64 + (int)((uint32_t)m >> 24) * kPrimBytes;
-      const unsigned char* __restrict__ src = p.units + (size_t)e * kUnitBytes + lane * 16;
+      const unsigned char* __restrict__ src = Ucp + (uint64_t)(uint32_t)e * (uint32_t)kUnitBytes;
       if (lane * 16 < nb) cp16(dst, src);
       if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
-      const double* __restrict__ Fsrc = Fc + (int64_t)(m & 0xffffff) * ld + pbase + lane * 2;
+      const char* __restrict__ Fsrc = Fcp + (uint64_t)(uint32_t)(m & 0xffffff) * ld8;
 #pragma unroll
       for (int k2 = 0; k2 < NB; ++k2)
 #pragma unroll
         for (int c = 0; c < NP * 16; c += 32)
-          if (c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (int64_t)k2 * ld + c * 2);
+          if (c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (uint64_t)k2 * ld8 + c * 16);
     }
     cp_commit();
   };
@@ -191,7 +200,6 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
   for (int k = 0; k < D; ++k) issue(k, e0, m0);
 
   int cur_fa = -1;
-  int64_t cur_offa = 0;
   double Fa[NP][NA], Ga[NP][NA];
 #pragma unroll
   for (int s = 0; s < NP; ++s)
@@ -203,7 +211,7 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
     for (int s = 0; s < NP; ++s)
       if (act[s]) {
 #pragma unroll
-        for (int i = 0; i < NA; ++i) atomicAdd(Gc + cur_offa + (int64_t)i * ld + pt[s], Ga[s][i]);
+        for (int i = 0; i < NA; ++i) G_add(cur_fa + i, s, Ga[s][i]);
       }
   };
 
@@ -219,15 +227,14 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
       const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
       ABx = ab0.x; ABy = ab0.y; ABz = *reinterpret_cast<const double*>(rec + 32);
     }
-    const longlong2 off = *reinterpret_cast<const longlong2*>(rec + 48);   // fa * ld, fb * ld
     if (fa != cur_fa) {
       if (cur_fa >= 0) flush_a();
-      cur_fa = fa; cur_offa = off.x;
+      cur_fa = fa;
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
         for (int i = 0; i < NA; ++i) {
-          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = Fc[off.x + (int64_t)i * ld + ptc[s]];
+          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = F_at(fa + i, s);
           Ga[s][i] = 0.0;
         }
     }
@@ -244,7 +251,7 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) Fa[s][i] = __ldg(Fc + cur_offa + (int64_t)i * ld + ptc[s]);
+        for (int i = 0; i < NA; ++i) Fa[s][i] = F_at(cur_fa + i, s);
     }
 #pragma unroll
     for (int s = 0; s < NP; ++s) {
@@ -261,7 +268,7 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
       for (int s = 0; s < NP; ++s)
         if (act[s]) {
 #pragma unroll
-          for (int k2 = 0; k2 < NB; ++k2) atomicAdd(Gc + off.y + (int64_t)k2 * ld + pt[s], Gb[s][k2]);
+          for (int k2 = 0; k2 < NB; ++k2) G_add(fb + k2, s, Gb[s][k2]);
         }
     }
   }
@@ -288,16 +295,17 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg;
   unsigned char* ring = smem_int + warp * (D * SLOT);
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
+  if (tile.n - pbase >= 32 * NPM) { consume_units<LA, LB, NPM, WPG, true>(p, tile, list, cnt, ring, pbase, rnk, lane); return; }
   if constexpr (NPM == 4) {
-    if (need == 4) consume_units<LA, LB, 4, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else if (need == 3) consume_units<LA, LB, 3, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    if (need == 4) consume_units<LA, LB, 4, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else if (need == 3) consume_units<LA, LB, 3, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else if (need == 2) consume_units<LA, LB, 2, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
   } else if constexpr (NPM == 2) {
-    if (need == 2) consume_units<LA, LB, 2, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    if (need == 2) consume_units<LA, LB, 2, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    else consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
   } else {
-    consume_units<LA, LB, 1, WPG>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
   }
 }
 

@@ -124,7 +124,13 @@ __host__ __device__ constexpr int boys_x2max_hi(int L) {       // high word of t
 }
 // x2 >= 2 xmax(L) for a non-negative finite double: an integer compare of the high words (the FP64 pipe is the scarce one)
 template <int L>
-__device__ __forceinline__ bool is_far(double x2) { return __double2hiint(x2) >= boys_x2max_hi(L); }
+__device__ __forceinline__ bool is_far(double x2) {
+#ifdef SNK_KNOCKOUT_NEAR           // timing experiment only (wrong integrals): what the near-field branch costs
+  return true;
+#else
+  return __double2hiint(x2) >= boys_x2max_hi(L);
+#endif
+}
 
 template <int L>
 __device__ __forceinline__ void seeds_far(double x2, double cfar2, double (&T)[L + 1]) {

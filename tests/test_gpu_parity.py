@@ -383,3 +383,17 @@ def test_sharded_build_on_one_gpu(snk_mod, oracle_mod, torch_cuda):
     assert abs(sum(loads) - costs.sum()) <= 0.01 * costs.sum()
     assert max(loads) <= 1.5 * np.mean(loads), loads                                # LPT balance on the work model
     print("shard loads (primitive pair-points):", ["%.3g" % x for x in loads])
+
+
+def test_K_decaying_density(snk_mod, oracle_mod):
+    """spatially decaying density (localised random orbitals, |P| ~ exp(-r / 0.8 bohr)) on the
+    27-water cluster with config 3's basis: Eq. 46 now localises, V_j loses pairs the dense density keeps, and the GPU and
+    the oracle must delete exactly the same ones (lists audited) and agree on K."""
+    kw = dict(grid=(8, 6, 8), lattice=3)
+    wd = inputs.make_workload(3, density="decay", decay_bohr=0.8, **kw)
+    _, _, ctx = _run_both(snk_mod, oracle_mod, wd, eps=1e-7, tag="decaying density")
+    sv_decay = ctx.stats()["sum_V"]
+    wf = inputs.make_workload(3, **kw)
+    assert np.array_equal(wf.points, wd.points)
+    _, _, ctx2 = _run_both(snk_mod, oracle_mod, wf, eps=1e-7, audit=False, tag="dense density, same grid")
+    assert sv_decay < 0.8 * ctx2.stats()["sum_V"], (sv_decay, ctx2.stats()["sum_V"])
