@@ -170,7 +170,8 @@ def _ncu_traffic(cfg, cls_name):
             col = {h.split("[")[0]: (i, (h.split("[")[1][:-1] if "[" in h else "")) for i, h in enumerate(hdr)}
             for r in rows[1:]:
                 if "k_integrals<%s>" % la_lb in r[col["kernel"][0]]:
-                    return sum(float(r[col[k][0]]) * scale.get(col[k][1], 1.0) for k in ("dram_read", "dram_write"))
+                    v = sum(float(r[col[k][0]]) * scale.get(col[k][1], 1.0) for k in ("dram_read", "dram_write"))
+                    return v if v == v else None          # ncu left the section empty for this launch
         except Exception:
             continue
     return None
