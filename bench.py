@@ -330,7 +330,9 @@ def main():
     roofline = {"bound": "alu", "kernel": "k_integrals<%s>" % snk.CLASS_NAMES[cls], "achieved": achieved, "peak": dfma_peak, "unit": "TFLOP/s",
                 "frac": achieved / dfma_peak if dfma_peak else None, "traffic": _ncu_traffic(args.config, snk.CLASS_NAMES[cls]),
                 "peak_source": "measured on this GPU by snk_measure_fp64_peak (register-resident DFMA loop); nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2",
-                "flops_per_launch": k_flops, "ms_per_launch": k_ms,
+                "launches_per_step": int(st["nsuper"]),     # one launch of every class per super-batch
+                "flops_per_launch": k_flops / max(1, st["nsuper"]), "ms_per_launch": k_ms / max(1, st["nsuper"]),
+                "traffic_note": "dram bytes read + written by the first of these launches in profiles/*_ncu_full_cfg<N>.csv (ncu --set full)",
                 "all_integral_kernels": {"achieved": st["flops_integral"] / (all_ms * 1e-3) * 1e-12 if all_ms > 0 else 0.0, "ms": all_ms,
                                          "flops": st["flops_integral"], "share_of_step": all_ms / st["ms_build"] if st["ms_build"] else None},
                 "gemm_dmma": {"peak": dmma_peak, "achieved": st["flops_gemm"] / ((st["ms_F"] + st["ms_Kt"] + 1e-12) * 1e-3) * 1e-12,
