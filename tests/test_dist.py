@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from paper_2303_14280_b200 import inputs
-from paper_2303_14280_b200.dist import lpt_partition, root_cell_keys, root_cell_sample, shard_points
+from paper_2303_14280_b200.dist import lpt_partition, root_cell_costs, root_cell_keys, root_cell_sample, shard_points
 
 
 def _free_port():
@@ -50,6 +50,37 @@ def test_shards_are_whole_root_cells_and_cover_the_grid():
         assert np.all(tot == 1)                                             # every point owned exactly once
     m = root_cell_sample(w.points, w.batch_cell, 0.2)
     assert 0 < m.sum() < len(key) and not (set(key[m].tolist()) & set(key[~m].tolist()))
+
+
+def test_cost_based_partition_balances_work_not_points(oracle_mod):
+    """Alg. 2 on a work model: per-batch costs (here the oracle's own pair counts times points, standing in for
+    snk_batch_costs, which needs a GPU) are summed per root cell and balance the partition better than point counts do."""
+    w = inputs.make_workload(2, grid=(8, 6, 8))
+    o = oracle_mod.Oracle(w.basis)
+    o.set_grid(w.points, w.weights, eps=w.eps, batch_cell=w.batch_cell, batch_max=256)
+    o.screen(w.P)
+    off, perm, _ = o.batches()
+    Voff, _ = o.V_lists()
+    costs = np.diff(off) * np.diff(Voff).astype(float)           # pair-points per batch
+    keys, cell_cost = root_cell_costs(w.points, w.batch_cell, off, perm, costs)
+    assert np.array_equal(keys, np.unique(root_cell_keys(w.points, w.batch_cell)))
+    assert abs(cell_cost.sum() - costs.sum()) <= 1e-9 * costs.sum()
+    key = root_cell_keys(w.points, w.batch_cell)
+    first = perm[off[:-1]]
+    for world in (2, 4):
+        def imbalance(cc):
+            load = np.zeros(world)
+            for r in range(world):
+                m = shard_points(w.points, w.batch_cell, r, world, cell_costs=cc)
+                assert not (set(key[m].tolist()) & set(key[~m].tolist()))                  # whole root cells
+                load[r] = costs[m[first]].sum()
+            assert abs(load.sum() - costs.sum()) <= 1e-9 * costs.sum()
+            return load.max() / load.mean()
+        by_cost, by_points = imbalance((keys, cell_cost)), imbalance(None)
+        assert by_cost <= by_points + 1e-12, (world, by_cost, by_points)
+        assert by_cost <= 1.0 + cell_cost.max() / (cell_cost.sum() / world)                # greedy bound: mean + largest task
+    with pytest.raises(AssertionError):
+        shard_points(w.points[:-7], w.batch_cell, 0, 2, cell_costs=(keys[:-1], cell_cost[:-1]))
 
 
 def _rank_main(rank, world, port, q):
