@@ -176,21 +176,21 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
   const unsigned char* __restrict__ Ucp = p.units + lane * 16;
   const char* __restrict__ Fcp = Fl + (pbase * 8 + lane * 16);
   const uint32_t dst_lane = s_ring + lane * 16;
-  // (no branch on k: the copies are predicated, so that the call can sit inside the straight-line block after a unit's loop)
   auto issue = [&](int k, int e_w, int m_w) {
-    const bool valid = k < n_my;
-    const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
-    const uint32_t dst = dst_lane + ((uint32_t)k % D) * SLOT;
-    const int nb = valid ? 64 + (int)((uint32_t)m >> 24) * kPrimBytes : 0;
-    const unsigned char* __restrict__ src = Ucp + (uint64_t)(uint32_t)e * (uint32_t)kUnitBytes;
-    if (lane * 16 < nb) cp16(dst, src);
-    if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
-    const char* __restrict__ Fsrc = Fcp + (uint64_t)(uint32_t)(m & 0xffffff) * ld8;
+    if (k < n_my) {
+      const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
+      const uint32_t dst = dst_lane + ((uint32_t)k % D) * SLOT;
+      const int nb = 64 + (int)((uint32_t)m >> 24) * kPrimBytes;
+      const unsigned char* __restrict__ src = Ucp + (uint64_t)(uint32_t)e * (uint32_t)kUnitBytes;
+      if (lane * 16 < nb) cp16(dst, src);
+      if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
+      const char* __restrict__ Fsrc = Fcp + (uint64_t)(uint32_t)(m & 0xffffff) * ld8;
 #pragma unroll
-    for (int k2 = 0; k2 < NB; ++k2)
+      for (int k2 = 0; k2 < NB; ++k2)
 #pragma unroll
-      for (int c = 0; c < NP * 16; c += 32)
-        if (valid && c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (uint64_t)k2 * ld8 + c * 16);
+        for (int c = 0; c < NP * 16; c += 32)
+          if (c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (uint64_t)k2 * ld8 + c * 16);
+    }
     cp_commit();
   };
   int e0, m0, e1, m1;
@@ -215,78 +215,62 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
       }
   };
 
-  // Software pipeline over the units: the header and the F_b values of unit k+1 are read from its slot, and the copies of
-  // unit k+D are issued, in the same straight-line block as the HRR / contraction / REDs of unit k, so that their latencies
-  // (LDS, shuffles, address arithmetic) are covered by that unit's FP64 work instead of forming a serial chain of their own.
-  struct Hdr { int fa, fb, np; double ABx, ABy, ABz; };
-  Hdr hn;                                                          // unit k+1 (next)
-  double Fbn[NP][NB];
-  auto read_hdr = [&](int k) {
-    const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
-    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
-    hn.fa = h0.x; hn.fb = h0.y; hn.np = h0.z;
-    hn.ABx = hn.ABy = hn.ABz = 0.0;
-    if constexpr (LB > 0) {
-      const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
-      hn.ABx = ab0.x; hn.ABy = ab0.y; hn.ABz = *reinterpret_cast<const double*>(rec + 32);
-    }
-    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
-#pragma unroll
-    for (int s = 0; s < NP; ++s)
-#pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2) Fbn[s][k2] = Fs[k2 * (32 * NP) + 32 * s + lane];
-  };
-  cp_wait<D - 1>();                                                // unit 0 has landed (this thread's copies ...
-  __syncwarp();                                                    // ... and those of the other lanes)
-  read_hdr(0);
-
 #pragma unroll 1
   for (int k = 0; k < n_my; ++k) {
-    const Hdr h = hn;
-    double Fb[NP][NB], Gb[NP][NB];
-#pragma unroll
-    for (int s = 0; s < NP; ++s)
-#pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2) { Fb[s][k2] = Fbn[s][k2]; Gb[s][k2] = 0.0; }
-    if (h.fa != cur_fa) {
+    cp_wait<D - 1>();                                              // this thread's copies of unit k have landed ...
+    __syncwarp();                                                  // ... and so have those of the other lanes
+    const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
+    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
+    const int fa = h0.x, fb = h0.y;
+    double ABx = 0.0, ABy = 0.0, ABz = 0.0;
+    if constexpr (LB > 0) {
+      const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
+      ABx = ab0.x; ABy = ab0.y; ABz = *reinterpret_cast<const double*>(rec + 32);
+    }
+    if (fa != cur_fa) {
       if (cur_fa >= 0) flush_a();
-      cur_fa = h.fa;
+      cur_fa = fa;
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
         for (int i = 0; i < NA; ++i) {
-          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = F_at(h.fa + i, s);
+          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = F_at(fa + i, s);
           Ga[s][i] = 0.0;
         }
     }
-    const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
+    double Fb[NP][NB], Gb[NP][NB];
+    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
+#pragma unroll
+    for (int s = 0; s < NP; ++s)
+#pragma unroll
+      for (int k2 = 0; k2 < NB; ++k2) { Fb[s][k2] = Fs[k2 * (32 * NP) + 32 * s + lane]; Gb[s][k2] = 0.0; }
+
     double acc[NP][nlev(LA, L)];
-    theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h.np, gx, gy, gz, p.boys, acc);
-    __syncwarp();                                                  // every lane is done with slot k % D
-    cp_wait<D - 2>();                                              // unit k+1 has landed (groups 0 .. D+k-1 are committed)
-    __syncwarp();
-    // ---- one straight-line block from here to the end of the iteration ----
+    theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
     if constexpr (int_fa_reload(LA, LB)) {
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
         for (int i = 0; i < NA; ++i) Fa[s][i] = F_at(cur_fa + i, s);
     }
-    read_hdr(k + 1);                                               // (past the end: a stale slot, never used)
 #pragma unroll
     for (int s = 0; s < NP; ++s) {
       ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
-      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], h.ABx, h.ABy, h.ABz, sink);
+      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ABx, ABy, ABz, sink);
     }
+
+    __syncwarp();                                                  // every lane is done with the slot: refill it D units ahead
     const int kn = k + D;
     if ((kn & 31) == 0 && kn < n_my) { e0 = e1; m0 = m1; load_win(kn + 32, e1, m1); }
-    issue(kn, e0, m0);                                             // refill slot k % D, D units ahead
-    const bool two_way = h.fa != h.fb;                             // a == b (same shell): one direction only
+    issue(kn, e0, m0);
+    if (fa != fb) {                                                // a == b (same shell): one direction only
 #pragma unroll
-    for (int s = 0; s < NP; ++s)
+      for (int s = 0; s < NP; ++s)
+        if (act[s]) {
 #pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2)
-        if (act[s] && two_way) G_add(h.fb + k2, s, Gb[s][k2]);
+          for (int k2 = 0; k2 < NB; ++k2) G_add(fb + k2, s, Gb[s][k2]);
+        }
+    }
   }
   if (cur_fa >= 0) flush_a();
 }
