@@ -728,6 +728,9 @@ static int build_impl(snk_ctx* ctx, const double* P, double* K, void* stream_, b
     ctx->n_launches += 1;
     ip.vlist = ctx->d_vlist.p; ip.vlstride = nunit; ip.vcnt = ctx->d_vcnt.p; ip.b0 = su.b0;
     ip.units = ctx->d_units.p; ip.meta = ctx->d_meta.p; ip.boys = ctx->d_boys.p;
+    // few tiles (large basis: the workspace holds few slots) would leave the last wave of a launch mostly empty: let several
+    // CTAs share a tile until there are some 4 000 CTAs (more than 8 waves of the 296-444 resident ones)
+    ip.nsplit = std::max(1, std::min(8, 4000 / std::max(1, ntiles)));
     for (int c = 0; c < kNumClasses; ++c) {
       ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1]; ip.cls = c;
       if (ip.pend <= ip.pbeg) continue;

@@ -132,13 +132,14 @@ __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0
 // FULL: every lane of the warp owns NP points of the tile (no predicates, no clamped indices); ragged groups take FULL = false.
 // Row addresses in the F / G slabs are base + row * ld8 with a 32-bit byte stride ld8 (the host keeps ld * 8 < 2^32): one
 // 32 x 32 -> 64 bit multiply-add per address.
-template <int LA, int LB, int NP, int WPG, bool FULL>
+// The warp takes the list entries rnk, rnk + stride, ... (stride = warps of the point group x CTAs that share the tile).
+template <int LA, int LB, int NP, bool FULL>
 __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec& tile, const int32_t* __restrict__ list, int cnt,
-                                              unsigned char* ring, int pbase, int rnk, int lane) {
+                                              unsigned char* ring, int pbase, int rnk, int stride, int lane) {
   constexpr int NA = ncart(LA), NB = ncart(LB), L = LA + LB;
   constexpr int D = int_depth(LA, LB), SLOT = int_slot_bytes(LB, int_npmax(LA, LB));
   constexpr uint32_t FROW = 32u * NP * 8u;             // bytes of one staged F row segment
-  const int n_my = cnt > rnk ? (cnt - rnk + WPG - 1) / WPG : 0;
+  const int n_my = cnt > rnk ? (cnt - rnk + stride - 1) / stride : 0;
   if (n_my == 0) return;
   const uint32_t s_ring = smem_u32(ring);
 
@@ -166,7 +167,7 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
     const int q = wb + lane;
     e = 0; m = 0;
     if (q < n_my) {
-      e = __ldg(list + (int64_t)q * WPG + rnk);
+      e = __ldg(list + (int64_t)q * stride + rnk);
       const int2 mm = __ldg(reinterpret_cast<const int2*>(&p.meta[e].fb));   // fb, nprim | first << 8
       m = mm.x | (mm.y & 0xff) << 24;
     }
@@ -285,27 +286,30 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
 
-  const TileRec tile = p.tiles[blockIdx.x];
+  // p.nsplit CTAs share a tile (launches with few tiles, e.g. a large basis on a small super-batch): CTA `part` takes every
+  // nsplit-th share of the unit list; G is accumulated with REDs anyway
+  const int tile_id = blockIdx.x / p.nsplit, part = blockIdx.x - tile_id * p.nsplit;
+  const TileRec tile = p.tiles[tile_id];
   const int jj = tile.batch - p.b0;
   const int cnt = p.vcnt[jj * kNumClasses + p.cls];                  // units of this class kept by the tile's batch
   if (cnt == 0) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int grp = warp / WPG, rnk = warp % WPG, pbase = grp * 32 * NPM;
+  const int grp = warp / WPG, rnk = part * WPG + warp % WPG, stride = WPG * p.nsplit, pbase = grp * 32 * NPM;
   if (pbase >= tile.n) return;
   const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg;
   unsigned char* ring = smem_int + warp * (D * SLOT);
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
-  if (tile.n - pbase >= 32 * NPM) { consume_units<LA, LB, NPM, WPG, true>(p, tile, list, cnt, ring, pbase, rnk, lane); return; }
+  if (tile.n - pbase >= 32 * NPM) { consume_units<LA, LB, NPM, true>(p, tile, list, cnt, ring, pbase, rnk, stride, lane); return; }
   if constexpr (NPM == 4) {
-    if (need == 4) consume_units<LA, LB, 4, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else if (need == 3) consume_units<LA, LB, 3, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else if (need == 2) consume_units<LA, LB, 2, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    if (need == 4) consume_units<LA, LB, 4, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
+    else if (need == 3) consume_units<LA, LB, 3, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
+    else if (need == 2) consume_units<LA, LB, 2, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
+    else consume_units<LA, LB, 1, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
   } else if constexpr (NPM == 2) {
-    if (need == 2) consume_units<LA, LB, 2, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
-    else consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    if (need == 2) consume_units<LA, LB, 2, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
+    else consume_units<LA, LB, 1, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
   } else {
-    consume_units<LA, LB, 1, WPG, false>(p, tile, list, cnt, ring, pbase, rnk, lane);
+    consume_units<LA, LB, 1, false>(p, tile, list, cnt, ring, pbase, rnk, stride, lane);
   }
 }
 
@@ -335,7 +339,7 @@ cudaError_t launch_class(const IntParams& p, cudaStream_t s) {
     constexpr int smem = int_smem_bytes(LA, LB);
     static bool attr_set[kMaxDevices] = {};
     if (cudaError_t e = opt_in_smem(k_integrals<LA, LB>, smem, attr_set); e != cudaSuccess) return e;
-    k_integrals<LA, LB><<<p.ntiles, int_threads(LA, LB), smem, s>>>(p);
+    k_integrals<LA, LB><<<p.ntiles * p.nsplit, int_threads(LA, LB), smem, s>>>(p);
   }
   return cudaGetLastError();
 }

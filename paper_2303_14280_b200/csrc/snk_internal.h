@@ -108,6 +108,7 @@ struct IntParams {
   const int32_t* vcnt;                      // [batches of the super-batch][kNumClasses] kept units per class
   int b0;                                   // first batch of the super-batch
   int cls;                                  // class of this launch
+  int nsplit;                               // CTAs per tile: each takes every nsplit-th share of the tile's unit list
   int pbeg, pend;          // range of this class in the unit list
   const unsigned char* units;               // [nunit][kUnitBytes]
   const UnitMeta* meta;                     // [nunit]
