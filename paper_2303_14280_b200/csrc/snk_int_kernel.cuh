@@ -177,28 +177,30 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
   const unsigned char* __restrict__ Ucp = p.units + lane * 16;
   const char* __restrict__ Fcp = Fl + (pbase * 8 + lane * 16);
   const uint32_t dst_lane = s_ring + lane * 16;
+  // (no branch on k: the copies are predicated)
   auto issue = [&](int k, int e_w, int m_w) {
-    if (k < n_my) {
-      const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
-      const uint32_t dst = dst_lane + ((uint32_t)k % D) * SLOT;
-      const int nb = 64 + (int)((uint32_t)m >> 24) * kPrimBytes;
-      const unsigned char* __restrict__ src = Ucp + (uint64_t)(uint32_t)e * (uint32_t)kUnitBytes;
-      if (lane * 16 < nb) cp16(dst, src);
-      if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
-      const char* __restrict__ Fsrc = Fcp + (uint64_t)(uint32_t)(m & 0xffffff) * ld8;
+    const bool valid = k < n_my;
+    const int e = __shfl_sync(0xffffffffu, e_w, k & 31), m = __shfl_sync(0xffffffffu, m_w, k & 31);
+    const uint32_t dst = dst_lane + ((uint32_t)k % D) * SLOT;
+    const int nb = valid ? 64 + (int)((uint32_t)m >> 24) * kPrimBytes : 0;
+    const unsigned char* __restrict__ src = Ucp + (uint64_t)(uint32_t)e * (uint32_t)kUnitBytes;
+    if (lane * 16 < nb) cp16(dst, src);
+    if (512 + lane * 16 < nb) cp16(dst + 512, src + 512);
+    const char* __restrict__ Fsrc = Fcp + (uint64_t)(uint32_t)(m & 0xffffff) * ld8;
 #pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2)
+    for (int k2 = 0; k2 < NB; ++k2)
 #pragma unroll
-        for (int c = 0; c < NP * 16; c += 32)
-          if (c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (uint64_t)k2 * ld8 + c * 16);
-    }
+      for (int c = 0; c < NP * 16; c += 32)
+        if (valid && c + lane < NP * 16) cp16(dst + kUnitBytes + k2 * FROW + c * 16, Fsrc + (uint64_t)k2 * ld8 + c * 16);
     cp_commit();
   };
   int e0, m0, e1, m1;
   load_win(0, e0, m0);
   load_win(32, e1, m1);
+  // units 0 .. D-2 are staged here; unit k+D-1 is staged at the top of iteration k, right after the one __syncwarp of the
+  // iteration (every lane is then done with unit k-1, whose slot it takes)
 #pragma unroll
-  for (int k = 0; k < D; ++k) issue(k, e0, m0);
+  for (int k = 0; k < D - 1; ++k) issue(k, e0, m0);
 
   int cur_fa = -1;
   double Fa[NP][NA], Ga[NP][NA];
@@ -216,62 +218,66 @@ __device__ __forceinline__ void consume_units(const IntParams& p, const TileRec&
       }
   };
 
+  // windows of 32 units: the id registers move on between windows, not inside the unit loop
 #pragma unroll 1
-  for (int k = 0; k < n_my; ++k) {
-    cp_wait<D - 1>();                                              // this thread's copies of unit k have landed ...
-    __syncwarp();                                                  // ... and so have those of the other lanes
-    const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
-    const int4 h0 = *reinterpret_cast<const int4*>(rec);           // fa, fb, nprim, first
-    const int fa = h0.x, fb = h0.y;
-    double ABx = 0.0, ABy = 0.0, ABz = 0.0;
-    if constexpr (LB > 0) {
-      const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
-      ABx = ab0.x; ABy = ab0.y; ABz = *reinterpret_cast<const double*>(rec + 32);
-    }
-    if (fa != cur_fa) {
-      if (cur_fa >= 0) flush_a();
-      cur_fa = fa;
+  for (int kw = 0; kw < n_my; kw += 32) {
+    const int kend = min(kw + 32, n_my);
+#pragma unroll 1
+    for (int k = kw; k < kend; ++k) {
+      cp_wait<D - 2>();                                            // this thread's copies of unit k have landed ...
+      __syncwarp();                                                // ... and so have the other lanes'; all are done with unit k-1
+      {
+        const int kn = k + D - 1;                                  // kn's window is the current one or the next
+        issue(kn, (kn & 32) == (kw & 32) ? e0 : e1, (kn & 32) == (kw & 32) ? m0 : m1);
+      }
+      const unsigned char* rec = ring + ((uint32_t)k % D) * SLOT;
+      const int4 h0 = *reinterpret_cast<const int4*>(rec);         // fa, fb, nprim, first
+      const int fa = h0.x, fb = h0.y;
+      double ABx = 0.0, ABy = 0.0, ABz = 0.0;
+      if constexpr (LB > 0) {
+        const double2 ab0 = *reinterpret_cast<const double2*>(rec + 16);
+        ABx = ab0.x; ABy = ab0.y; ABz = *reinterpret_cast<const double*>(rec + 32);
+      }
+      if (fa != cur_fa) {
+        if (cur_fa >= 0) flush_a();
+        cur_fa = fa;
+#pragma unroll
+        for (int s = 0; s < NP; ++s)
+#pragma unroll
+          for (int i = 0; i < NA; ++i) {
+            if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = F_at(fa + i, s);
+            Ga[s][i] = 0.0;
+          }
+      }
+      double Fb[NP][NB], Gb[NP][NB];
+      const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) {
-          if constexpr (!int_fa_reload(LA, LB)) Fa[s][i] = F_at(fa + i, s);
-          Ga[s][i] = 0.0;
-        }
-    }
-    double Fb[NP][NB], Gb[NP][NB];
-    const double* Fs = reinterpret_cast<const double*>(rec + kUnitBytes);
-#pragma unroll
-    for (int s = 0; s < NP; ++s)
-#pragma unroll
-      for (int k2 = 0; k2 < NB; ++k2) { Fb[s][k2] = Fs[k2 * (32 * NP) + 32 * s + lane]; Gb[s][k2] = 0.0; }
+        for (int k2 = 0; k2 < NB; ++k2) { Fb[s][k2] = Fs[k2 * (32 * NP) + 32 * s + lane]; Gb[s][k2] = 0.0; }
 
-    double acc[NP][nlev(LA, L)];
-    theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
-    if constexpr (int_fa_reload(LA, LB)) {
+      double acc[NP][nlev(LA, L)];
+      theta_contracted<LA, LB, NP, true>(reinterpret_cast<const PrimPair*>(rec + 64), h0.z, gx, gy, gz, p.boys, acc);
+      if constexpr (int_fa_reload(LA, LB)) {
+#pragma unroll
+        for (int s = 0; s < NP; ++s)
+#pragma unroll
+          for (int i = 0; i < NA; ++i) Fa[s][i] = F_at(cur_fa + i, s);
+      }
+#pragma unroll
+      for (int s = 0; s < NP; ++s) {
+        ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
+        HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ABx, ABy, ABz, sink);
+      }
+      const bool two_way = fa != fb;                               // a == b (same shell): one direction only
 #pragma unroll
       for (int s = 0; s < NP; ++s)
 #pragma unroll
-        for (int i = 0; i < NA; ++i) Fa[s][i] = F_at(cur_fa + i, s);
+        for (int k2 = 0; k2 < NB; ++k2)
+          if (act[s] && two_way) G_add(fb + k2, s, Gb[s][k2]);
     }
-#pragma unroll
-    for (int s = 0; s < NP; ++s) {
-      ContractSink<LA, LB> sink{Fa[s], Fb[s], Ga[s], Gb[s]};
-      HrrNode<LA, LB, 0, 0, 0, L>::run(acc[s], ABx, ABy, ABz, sink);
-    }
-
-    __syncwarp();                                                  // every lane is done with the slot: refill it D units ahead
-    const int kn = k + D;
-    if ((kn & 31) == 0 && kn < n_my) { e0 = e1; m0 = m1; load_win(kn + 32, e1, m1); }
-    issue(kn, e0, m0);
-    if (fa != fb) {                                                // a == b (same shell): one direction only
-#pragma unroll
-      for (int s = 0; s < NP; ++s)
-        if (act[s]) {
-#pragma unroll
-          for (int k2 = 0; k2 < NB; ++k2) G_add(fb + k2, s, Gb[s][k2]);
-        }
-    }
+    e0 = e1; m0 = m1;
+    load_win(kw + 64, e1, m1);
   }
   if (cur_fa >= 0) flush_a();
 }
@@ -282,7 +288,7 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   constexpr int WPG = CW * NPM * 32 / kTile;                         // warps per point group
   static_assert(WPG >= 1 && WPG * (kTile / (32 * NPM)) == CW, "warps: a whole number per point group");
   constexpr int D = int_depth(LA, LB), SLOT = int_slot_bytes(LB, NPM);
-  static_assert((D & (D - 1)) == 0, "ring depth");
+  static_assert((D & (D - 1)) == 0 && D >= 2 && D <= 32, "ring depth");
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
 

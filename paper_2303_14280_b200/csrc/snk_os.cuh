@@ -445,8 +445,14 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
 #pragma unroll 1
     for (; k + KP <= nprim; k += KP) step(std::integral_constant<int, KP>{}, k);
   }
+  if constexpr (WARP && KP == 1) {
+    // the build kernel never sees a unit without primitive pairs (such units are not in V_j): no entry test
 #pragma unroll 1
-  for (; k < nprim; ++k) step(std::integral_constant<int, 1>{}, k);
+    do { step(std::integral_constant<int, 1>{}, k); } while (++k < nprim);
+  } else {
+#pragma unroll 1
+    for (; k < nprim; ++k) step(std::integral_constant<int, 1>{}, k);
+  }
 }
 
 }  // namespace snk
