@@ -39,7 +39,7 @@ namespace snk {
 #define SNK_NP_L2 2
 #endif
 #ifndef SNK_NP_L3
-#define SNK_NP_L3 1
+#define SNK_NP_L3 2
 #endif
 __host__ __device__ constexpr int int_npmax(int LA, int LB) {
   const int L = LA + LB;
@@ -56,7 +56,7 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
 #define SNK_MB_L2 3
 #endif
 #ifndef SNK_MB_L3
-#define SNK_MB_L3 3
+#define SNK_MB_L3 2
 #endif
 #ifndef SNK_MB_L4
 #define SNK_MB_L4 1
