@@ -4,7 +4,8 @@
 //
 // B200 design (differs from the paper's A100 kernel):
 //   * the V_j bit masks are expanded once per super-batch into per-(batch, class) unit-id lists (k_vlist); the warps of a tile
-//     that cover the same points (a point group: 4 of the 8 warps for L <= 1, 2 for L = 2) take the list's entries round robin;
+//     that cover the same points (a point group: the 8 warps for s-s, 4 of 8 for L = 1, 2 of 4 for L = 2, 3) take the list's
+//     entries round robin; when a launch has few tiles, several CTAs share a tile and split its list the same way;
 //   * every warp streams ITS units -- header + primitive pairs (<= 704 B) and the F_b row segments of its points -- through a
 //     private ring of D shared-memory slots with 16-byte cp.async copies, one commit group per unit: the warp refills a slot as
 //     soon as it has finished the unit in it, D units ahead, so the recurrences run against broadcast LDS only and never wait
@@ -12,8 +13,8 @@
 //     allocated in warp pairs), no tickets, no barrier shared between warps.  (Bulk copies completing on mbarriers were
 //     measured first: one elected lane pays ~60 instructions per unit for the uniform-register set-up of 1 + ncart(l_b) copies;
 //     the per-lane 16-byte copies cost a fifth of that and need no barrier objects.);
-//   * a thread owns NP points of the tile (2 for L <= 1, else 1): the point-independent work of a unit is paid once per 32 NP
-//     points and the NP recurrences are independent instruction streams;
+//   * a thread owns NP points of the tile (4 for s-s, 2 for L = 1..3, else 1): the point-independent work of a unit is paid
+//     once per 32 NP points and the NP recurrences are independent instruction streams;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
 //     fire-and-forget RED.F64 (coalesced along the slot index);
 //   * recurrence intermediates live in registers (compile-time unrolled VRR/HRR, snk_os.cuh).
@@ -24,11 +25,11 @@
 
 namespace snk {
 
-// Work split inside a CTA (one tile of up to kTile points, four consumer warps + one producer warp).
-// A consumer thread holds NP = int_npmax points of the tile (lane, lane + 32, ...): everything that does not depend on the grid
-// point -- the broadcast LDS of the primitive pairs, the loop and barrier bookkeeping -- is paid once per NP points, and the
-// NP recurrences are independent instruction streams.  The tile is therefore covered by G = 4 / NP point groups of NP warps
-// each, and the warps of one group share the unit stream: each takes the next unit nobody of its group has taken yet.
+// Work split inside a CTA (one tile of up to kTile points, CW warps).
+// A thread holds NP = int_npmax points of the tile (lane, lane + 32, ...): everything that does not depend on the grid
+// point -- the broadcast LDS of the primitive pairs, the loop and copy bookkeeping -- is paid once per NP points, and the
+// NP recurrences are independent instruction streams.  The tile is therefore covered by 4 / NP point groups of
+// WPG = CW NP / 4 warps each, and the warps of one group split the unit list round robin.
 #ifndef SNK_NP_L0
 #define SNK_NP_L0 4
 #endif
