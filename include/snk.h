@@ -143,6 +143,21 @@ int snk_debug_boys(int32_t mmax, int64_t n, const double* x, double* out, void* 
  * out DEVICE [n * ncart(l_a) * ncart(l_b)], row-major [g][ia][ib]. */
 int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double* pts, double* out, void* stream);
 
+/* ---- the same A block without any allocation --------------------------------------------------------
+ * snk_debug_A_pair cudaMallocs and frees a scratch buffer (the primitive-pair records of the shell pair) on every call and
+ * synchronises the stream.  Callers that cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it -- use this variant: same kernel, same arguments, same result layout (pts DEVICE [n*3] ->
+ * out DEVICE [n * ncart(l_a) * ncart(l_b)], row-major [g][ia][ib]), but the scratch is a fixed array inside the library
+ * (1024 primitive pairs x 80 bytes = 80 KB of device memory per GPU that loads the library, held until exit) that a small
+ * kernel fills on the device.  The call makes no cudaMalloc / cudaFree / allocating library call, copies nothing through
+ * the host and does not synchronise: it is ordered on `stream`, out is valid when the stream reaches the end of its work.
+ * LIMIT: nprim(a) * nprim(b) <= 1024, else SNK_EINVAL with the reason in snk_last_error.
+ * SHARED STATE: every call on a GPU uses the same scratch array, which keeps the last call's contents (each call overwrites
+ * the entries it reads; nothing needs clearing).  Calls that may overlap on the GPU (different streams, or concurrent
+ * graph branches) race on it: keep them on one stream or order them with events.
+ * Errors: SNK_EINVAL (bad shell index, NULL pointer, limit), SNK_ESTATE (wrong current device), SNK_ECUDA. */
+int snk_A_pair_noalloc(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double* pts, double* out, void* stream);
+
 /* ---- measured FP64 roofs of this GPU: register-resident DFMA loop and DMMA.884 loop,
  * TFLOP/s each (2 flops per FMA), best of `reps`. */
 int snk_measure_fp64_peak(double* dfma_tflops, double* dmma_tflops, int32_t reps);

@@ -259,6 +259,53 @@ int guarded(snk_ctx* ctx, F&& body) {
 
 }  // namespace
 
+// ---- snk_A_pair_noalloc: the A-block kernel with its primitive-pair scratch in a file-scope device array ------------------
+// snk_debug_A_pair cudaMallocs (and frees) a buffer for the primitive-pair records of the shell pair on every call.  Callers
+// that must not allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc) get the same kernel with
+// that scratch here: kNoAllocMaxPrims records of 80 bytes = 80 KB, held by every GPU that loads the library until exit.
+// In host code `g_noalloc_prims` is only a host-side stand-in for the symbol: its device address comes from
+// cudaGetSymbolAddress (noalloc_scratch, once per device, with that device current) and only that pointer goes to kernels.
+constexpr int kNoAllocMaxPrims = 1024;
+static __device__ __align__(256) unsigned char g_noalloc_prims[kNoAllocMaxPrims * kPrimBytes];
+static_assert(sizeof(PrimPair) == kPrimBytes, "PrimPair layout");
+
+namespace {
+PrimPair* g_noalloc_ptr[kMaxDevices] = {};
+
+cudaError_t noalloc_scratch(int dev, PrimPair** out) {          // `dev` is the current device
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_prims);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[dev] = static_cast<PrimPair*>(p);
+  }
+  *out = g_noalloc_ptr[dev];
+  return cudaSuccess;
+}
+
+// primitive-pair records of shell pair (sa, sb), k-major like the host loop of snk_debug_A_pair (R1: prefactor restored).
+// Overwrites entries [0, nprim(sa) nprim(sb)) of the scratch; nothing has to start at zero.
+__global__ void k_noalloc_prims(ShellTab sh, int sa, int sb, PrimPair* __restrict__ out) {
+  const int npa = sh.nprim[sa], npb = sh.nprim[sb];
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= npa * npb) return;
+  const int k = t / npb, l = t - k * npb;
+  const double A[3] = {sh.cx[sa], sh.cy[sa], sh.cz[sa]}, B[3] = {sh.cx[sb], sh.cy[sb], sh.cz[sb]};
+  const double dx = A[0] - B[0], dy = A[1] - B[1], dz = A[2] - B[2];
+  const double AB2 = dx * dx + dy * dy + dz * dz;
+  const double za = sh.pexp[sh.poff[sa] + k], zb = sh.pexp[sh.poff[sb] + l];
+  const double ps = za + zb;
+  PrimPair q;
+  q.p2 = 2.0 * ps; q.inv2p = 0.5 / ps;
+  q.Px = (za * A[0] + zb * B[0]) / ps; q.Py = (za * A[1] + zb * B[1]) / ps; q.Pz = (za * A[2] + zb * B[2]) / ps;
+  q.PAx = q.Px - A[0]; q.PAy = q.Py - A[1]; q.PAz = q.Pz - A[2];
+  q.pref = sh.pcoef[sh.poff[sa] + k] * sh.pcoef[sh.poff[sb] + l] * (6.283185307179586 / ps) * exp(-(za * zb / ps) * AB2);
+  q.cfar2 = 1.2533141373155002512 * q.pref;
+  out[t] = q;
+}
+}  // namespace
+
 // ====================================================================================================================
 extern "C" {
 
@@ -956,6 +1003,28 @@ int snk_debug_A_pair(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double
   cudaError_t e2 = cudaStreamSynchronize(s);
   d.release();
   CK(e); CK(e2);
+  return SNK_OK;
+  });
+}
+
+int snk_A_pair_noalloc(snk_ctx* ctx, int32_t a, int32_t b, int64_t n, const double* pts, double* out, void* stream_) {
+  return guarded(ctx, [&]() -> int {
+  if (!ctx) return SNK_EINVAL;
+  if (a < 0 || b < 0 || a >= ctx->nsh || b >= ctx->nsh || n < 0 || (n > 0 && (!pts || !out))) FAIL(SNK_EINVAL, "snk_A_pair_noalloc: bad argument");
+  CHECK_DEVICE();
+  cudaStream_t s = (cudaStream_t)stream_;
+  const bool tr = ctx->h_l[a] < ctx->h_l[b];
+  const int sa = tr ? b : a, sb = tr ? a : b;
+  const int np = ctx->h_nprim[sa] * ctx->h_nprim[sb];
+  if (np > kNoAllocMaxPrims)
+    FAIL(SNK_EINVAL, "snk_A_pair_noalloc: the shell pair has more than 1024 primitive pairs (the fixed scratch); use snk_debug_A_pair");
+  PrimPair* scratch = nullptr;
+  CK(noalloc_scratch(ctx->device, &scratch));
+  if (n == 0) return SNK_OK;
+  k_noalloc_prims<<<(np + 127) / 128, 128, 0, s>>>(ctx->tab(), sa, sb, scratch);
+  CK(cudaGetLastError());
+  const double AB[3] = {ctx->h_cx[sa] - ctx->h_cx[sb], ctx->h_cy[sa] - ctx->h_cy[sb], ctx->h_cz[sa] - ctx->h_cz[sb]};
+  CK(launch_debug_A(ctx->h_l[sa], ctx->h_l[sb], tr, scratch, np, AB[0], AB[1], AB[2], pts, n, ctx->d_boys.p, out, s));
   return SNK_OK;
   });
 }

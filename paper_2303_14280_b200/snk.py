@@ -18,7 +18,7 @@ HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "snk.h")
 SNK_OK, SNK_EINVAL, SNK_ENOMEM, SNK_ECUDA, SNK_ESTATE = 0, -1, -2, -3, -4
 
 EXPORTS = ["snk_create", "snk_set_option", "snk_set_grid", "snk_build_K", "snk_build_K_host", "snk_screen", "snk_batch_costs", "snk_nbf", "snk_get_stats",
-           "snk_export_lists", "snk_debug_boys", "snk_debug_A_pair", "snk_measure_fp64_peak", "snk_last_error", "snk_destroy",
+           "snk_export_lists", "snk_debug_boys", "snk_debug_A_pair", "snk_A_pair_noalloc", "snk_measure_fp64_peak", "snk_last_error", "snk_destroy",
            "snk_version"]
 
 CLASS_NAMES = ["ss", "ps", "pp", "ds", "dp", "dd", "fs", "fp", "fd", "ff"]
@@ -74,6 +74,7 @@ def load():
     lib.snk_export_lists.argtypes = [vp, lp, lp, lp, lp, ip, lp, ip]
     lib.snk_debug_boys.argtypes = [C.c_int32, C.c_int64, vp, vp, vp]
     lib.snk_debug_A_pair.argtypes = [vp, C.c_int32, C.c_int32, C.c_int64, vp, vp, vp]
+    lib.snk_A_pair_noalloc.argtypes = [vp, C.c_int32, C.c_int32, C.c_int64, vp, vp, vp]
     lib.snk_measure_fp64_peak.argtypes = [dp, dp, C.c_int32]
     lib.snk_last_error.argtypes = [vp]
     lib.snk_last_error.restype = C.c_char_p
@@ -208,6 +209,15 @@ class Snk:
         n = pts.shape[0]
         out = torch.empty((n, self._nc(a), self._nc(b)), dtype=torch.float64, device=pts.device)
         self._check(self._lib.snk_debug_A_pair(self.h, int(a), int(b), int(n), _ptr(pts), _ptr(out), _stream(stream)))
+        return out
+
+    def A_pair_noalloc(self, a: int, b: int, pts, out, stream=None):
+        """snk_A_pair_noalloc: like debug_A_pair, but the caller passes ``out`` (CUDA float64 [n, ncart(l_a), ncart(l_b)]) and
+        the library allocates nothing; asynchronous on the stream."""
+        assert pts.is_cuda and pts.is_contiguous() and pts.element_size() == 8
+        n = pts.shape[0]
+        assert out.is_cuda and out.is_contiguous() and out.element_size() == 8 and out.numel() == n * self._nc(a) * self._nc(b)
+        self._check(self._lib.snk_A_pair_noalloc(self.h, int(a), int(b), int(n), _ptr(pts), _ptr(out), _stream(stream)))
         return out
 
     def _nc(self, s):
