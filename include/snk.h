@@ -90,7 +90,9 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
  *   "batch_cell"   h0, root cell edge of the lattice-anchored octree in bohr (R13). default 6.0
  *   "batch_max"    N_max, largest batch (R13), 32..4096.                           default 2048
  *   "workspace_gb" device-memory budget for the Phi/F/G super-batch (Alg. 1 l.8).  default 24
- *   "atomics"      1: G accumulated with RED.F64 (default); reserved.
+ *   "atomics"      1: G and the split-K partial tiles of Kt are accumulated with fp64 RED atomics (default, the only mode);
+ *                  the order of those additions is not fixed, so K is reproducible from run to run only up to fp64
+ *                  summation order (observed: a few 1e-15 relative), never bit for bit.  Reserved for a deterministic mode.
  * Must be set before snk_set_grid.  Unknown key or out-of-range value: SNK_EINVAL. */
 int snk_set_option(snk_ctx* ctx, const char* key, double value);
 
