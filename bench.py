@@ -81,9 +81,24 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def _morton_order(pts, h0):
+    """Order of the points along a Morton (Z-order) curve inside their root cells: a prefix of it is a spatially compact piece of
+    the grid, which the oracle's octree turns into batches of the usual size and shape."""
+    cell = np.floor(pts / h0)
+    q = np.clip(((pts / h0 - cell) * 1024.0).astype(np.int64), 0, 1023)
+    key = np.zeros(len(pts), dtype=np.int64)
+    for b in range(10):
+        for ax in range(3):
+            key |= ((q[:, ax] >> b) & 1) << (3 * b + ax)
+    ck = (cell[:, 0].astype(np.int64) + (1 << 15)) << 32 | (cell[:, 1].astype(np.int64) + (1 << 15)) << 16 | (cell[:, 2].astype(np.int64) + (1 << 15))
+    return np.lexsort((key, ck))
+
+
 def time_oracle_sample(w, target_s=15.0, first_frac=0.01, return_idx=False):
-    """Oracle (as it stands) on a bounded sample sized for ~target_s of host time: whole root cells in R13 hash order; when even
-    the first cells are too much (config 4: 3.3e6 integrals per point) every k-th point of them."""
+    """Oracle (as it stands) on a bounded sample sized for ~target_s of host time.  Whole root cells in R13 hash order when the
+    budget covers at least the first of them (they hold 5e4-1e5 points each in configs 3-5); otherwise a spatially compact part
+    of the first root cells (a Morton-order prefix: whole octree leaves, i.e. batches of the usual size), never scattered
+    points -- a batch with a handful of points pays the whole per-batch screening and would make the oracle look 10x slower."""
     from oracle import oracle as orc
     from paper_2303_14280_b200.dist import root_cell_sample
     o = orc.Oracle(w.basis)
@@ -95,27 +110,38 @@ def time_oracle_sample(w, target_s=15.0, first_frac=0.01, return_idx=False):
         o.build_K(w.P)
         return time.time() - t, o.stats()
 
-    idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, first_frac))[0] if first_frac < 1.0 else np.arange(npts)
-    probe = idx[::max(1, len(idx) // 128)]
-    dt0, _ = run(probe)
-    want = int(target_s * len(probe) / max(dt0, 1e-4))            # points the oracle can do in target_s
-    how = "whole root cells (R13 hash order)"
-    if want < len(idx):
-        idx = idx[::max(1, -(-len(idx) // max(want, 1)))]
-        how = "every k-th point of the first root cells (R13 hash order)"
-    elif want > 1.5 * len(idx) and first_frac < 1.0:
-        frac = min(1.0, first_frac * want / len(idx))
+    cells = np.nonzero(root_cell_sample(w.points, w.batch_cell, first_frac))[0] if first_frac < 1.0 else np.arange(npts)
+    cells = cells[_morton_order(w.points[cells], w.batch_cell)]
+    nprobe = min(len(cells), 256)
+    dt0, _ = run(cells[:nprobe])
+    want = int(target_s * nprobe / max(dt0, 1e-4))                # points the oracle can do in target_s
+    if want >= len(cells):
+        how = "whole root cells (R13 hash order)"
+        frac = min(1.0, first_frac * want / len(cells))
         idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, frac))[0] if frac < 1.0 else np.arange(npts)
+        if len(idx) > 1.3 * want:                                 # the next whole cell overshoots the budget: stay with the first ones
+            idx = cells
+    else:
+        how = "spatially compact part (Morton-order prefix, whole octree leaves) of the first root cells (R13 hash order)"
+        idx = cells[:max(want, nprobe)]
     dt, st = run(idx)
-    if dt < 0.6 * target_s and len(idx) < npts and how.startswith("whole"):      # the probe's rate was pessimistic: one more pass
-        frac = min(1.0, len(idx) / npts * target_s / max(dt, 1e-3))
-        idx = np.nonzero(root_cell_sample(w.points, w.batch_cell, frac))[0] if frac < 1.0 else np.arange(npts)
-        dt, st = run(idx)
+    if dt < 0.5 * target_s and len(idx) < npts:                   # the probe's rate was pessimistic: one more pass
+        want = int(len(idx) * target_s / max(dt, 1e-3))
+        if how.startswith("whole"):
+            frac = min(1.0, want / npts)
+            idx2 = np.nonzero(root_cell_sample(w.points, w.batch_cell, frac))[0] if frac < 1.0 else np.arange(npts)
+        else:
+            idx2 = cells[:min(want, len(cells))]
+        if len(idx2) > len(idx) and len(idx2) <= 1.5 * want:
+            idx = idx2
+            dt, st = run(idx)
     extra = {"idx": idx} if return_idx else {}
-    return dict(extra, value=st["n_int_contracted"] / dt, unit=UNIT, cores=st["threads"], kind="oracle",
-                sample="%s: %d of %d points (%.3f%%), %.3g contracted integrals, %.2f s; "
-                       "oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned" % (how, len(idx), npts, 100.0 * len(idx) / npts,
-                                                                                  st["n_int_contracted"], dt),
+    nb = len(o.batches()[0]) - 1
+    used = int(min(st["threads"], max(nb, 1)))                    # the oracle is parallel over batches: threads that had work
+    return dict(extra, value=st["n_int_contracted"] / dt, unit=UNIT, cores=used, kind="oracle",
+                sample="%s: %d of %d points (%.3f%%) in %d batches on %d OpenMP threads (parallel over batches: %d had work), "
+                       "%.3g contracted integrals, %.2f s; oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned"
+                       % (how, len(idx), npts, 100.0 * len(idx) / npts, nb, st["threads"], used, st["n_int_contracted"], dt),
                 seconds=dt, n_int=st["n_int_contracted"])
 
 
@@ -149,7 +175,7 @@ def run_reference(args, rank, world):
             "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": _workload_name(args.config, w), "sample": sample, "density": args.density, "batch_cell": w.batch_cell, "batch_max": w.batch_max},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": st["threads"], "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": first["cores"], "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
@@ -200,7 +226,7 @@ def main():
                     help="'dense' = BASELINE.json's P = C C^T with Gaussian C (no spatial decay: V_j keeps every significant pair); "
                          "'decay' = localised random orbitals, |P| ~ exp(-r / 1.5 bohr) (SURVEY.md section 8(f)-2: sn-LinK deletes work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--cpu-seconds", type=float, default=25.0, help="host time the oracle sample of cpu_baseline / --impl reference is sized for")
     ap.add_argument("--workspace-gb", type=float, default=None)
     ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
                     help="N>1: 'replicas' = every rank builds K for its own density (independent problems, no collective, weak scaling); "
