@@ -179,6 +179,35 @@ __device__ __forceinline__ void seeds_far_v(const double (&x2)[N], const double 
     }
   }
 }
+// the same with the hardware seed y0 ~ 1/sqrt(x2) already formed (it is issued before the far/near vote, off the critical path)
+template <int L, int N>
+__device__ __forceinline__ void seeds_far_v_y0(const double (&x2)[N], const double (&y0)[N], const double (&cfar2)[N], double (&T)[N][L + 1]) {
+  double e[N], u[N], r[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) u[i] = y0[i] * y0[i];
+#pragma unroll
+  for (int i = 0; i < N; ++i) e[i] = fma(-x2[i], u[i], 1.0);
+#pragma unroll
+  for (int i = 0; i < N; ++i) u[i] = y0[i] * e[i];
+#pragma unroll
+  for (int i = 0; i < N; ++i) e[i] = fma(e[i], 0.375, 0.5);
+#pragma unroll
+  for (int i = 0; i < N; ++i) r[i] = fma(e[i], u[i], y0[i]);
+#pragma unroll
+  for (int i = 0; i < N; ++i) T[i][0] = cfar2[i] * r[i];
+  if constexpr (L > 0) {
+    double h[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) h[i] = r[i] * r[i];
+#pragma unroll
+    for (int i = 0; i < N; ++i) T[i][1] = T[i][0] * h[i];
+#pragma unroll
+    for (int m = 1; m < L; ++m) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) T[i][m + 1] = T[i][m] * ((2 * m + 1) * h[i]);
+    }
+  }
+}
 template <int L>
 __device__ __forceinline__ void seeds_near(double x, double pref, const double* __restrict__ tab, double (&T)[L + 1]) {
   const double tm = fma(x, 16.0, 6755399441055744.0);
@@ -404,6 +433,14 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
     for (int i = 0; i < N; ++i) x[i] = fma(PCx[i], PCx[i], x[i]);
 #pragma unroll
     for (int i = 0; i < N; ++i) x[i] *= q0[i / NP].x;
+    // L <= 1: the hardware seed of 1/sqrt(2x) is issued before the far/near vote, so that its latency overlaps the vote's
+    // (measured: ss and ps -1.5 %, pp and above +1 %, hence the condition); near-field lanes do not use it
+    constexpr bool HOIST = WARP && L <= 1;
+    [[maybe_unused]] double y0[HOIST ? N : 1];
+    if constexpr (HOIST) {
+#pragma unroll
+      for (int i = 0; i < N; ++i) asm volatile("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0[i]) : "d"(x[i]));
+    }
     bool far = true;                                  // x[] holds 2x (p2 = 2p)
 #pragma unroll
     for (int i = 0; i < N; ++i) far = far && is_far<L>(x[i]);
@@ -416,7 +453,8 @@ __device__ __forceinline__ void theta_contracted(const PrimPair* __restrict__ pp
       double cf[N];
 #pragma unroll
       for (int i = 0; i < N; ++i) cf[i] = q4[i / NP].y;
-      seeds_far_v<L, N>(x, cf, th0);
+      if constexpr (HOIST) seeds_far_v_y0<L, N>(x, y0, cf, th0);
+      else seeds_far_v<L, N>(x, cf, th0);
     } else {
       // chain by chain: a chain whose 32 points are all far still runs without branches or table loads
 #pragma unroll
