@@ -228,6 +228,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=25.0, help="host time the oracle sample of cpu_baseline / --impl reference is sized for")
     ap.add_argument("--workspace-gb", type=float, default=None)
+    ap.add_argument("--tile-split", type=int, default=0, help="CTAs per tile in the integral kernel (0 = the library's choice)")
     ap.add_argument("--multi", default="replicas", choices=["replicas", "shard"],
                     help="N>1: 'replicas' = every rank builds K for its own density (independent problems, no collective, weak scaling); "
                          "'shard' = root cells dealt to ranks + NCCL all-reduce of K (Alg. 1/2, strong scaling)")
@@ -270,6 +271,8 @@ def main():
     s.set_option("eps", w.eps); s.set_option("batch_cell", w.batch_cell); s.set_option("batch_max", w.batch_max)
     if args.workspace_gb:
         s.set_option("workspace_gb", args.workspace_gb)
+    if args.tile_split:
+        s.set_option("tile_split", args.tile_split)
     dfma_peak, dmma_peak = snk.measure_fp64_peak(5)
     if shard:
         # Alg. 2 on the library's own work model: one screening pass over the whole grid gives the primitive

@@ -90,6 +90,8 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
  *   "batch_cell"   h0, root cell edge of the lattice-anchored octree in bohr (R13). default 6.0
  *   "batch_max"    N_max, largest batch (R13), 32..4096.                           default 2048
  *   "workspace_gb" device-memory budget for the Phi/F/G super-batch (Alg. 1 l.8).  default 24
+ *   "tile_split"   CTAs that share one 128-point tile in the integral kernel (each takes a contiguous share of the tile's
+ *                  unit list); 0 = the library's choice.                                     default 0
  *   "atomics"      1: G and the split-K partial tiles of Kt are accumulated with fp64 RED atomics (default, the only mode);
  *                  the order of those additions is not fixed, so K is reproducible from run to run only up to fp64
  *                  summation order (observed: a few 1e-15 relative), never bit for bit.  Reserved for a deterministic mode.

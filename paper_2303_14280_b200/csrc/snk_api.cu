@@ -36,6 +36,8 @@ struct snk_ctx {
   // options
   double eps = 0.0, h0 = 6.0, workspace_gb = 24.0;
   int nmax = 2048;
+  int tile_split = 0;           // CTAs per tile in a5; 0 = automatic
+  int sm_count = 148;
   // grid state
   bool have_grid = false;
   int64_t npts = 0, npts_kept = 0, nslots = 0, ldj = 0, ld = 0;
@@ -346,6 +348,7 @@ int snk_create(snk_ctx** out, int32_t natoms, const double* atom_xyz, int32_t ns
   if (!ctx) { g_create_error = "snk_create: out of host memory"; return SNK_ENOMEM; }
   auto bail = [&](int code, const std::string& m) { g_create_error = m; snk_destroy(ctx); ctx = nullptr; return code; };
   if (cudaGetDevice(&ctx->device) != cudaSuccess) return bail(SNK_ECUDA, "snk_create: no current CUDA device");
+  if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess || ctx->sm_count < 1) ctx->sm_count = 148;
   ctx->natoms = natoms; ctx->nsh = nshells;
   int64_t po = 0;
   int fo = 0;
@@ -437,6 +440,7 @@ int snk_set_option(snk_ctx* ctx, const char* key, double value) {
   else if (k == "batch_cell") { if (!(value > 0.0) || !std::isfinite(value)) FAIL(SNK_EINVAL, "batch_cell must be > 0"); ctx->h0 = value; }
   else if (k == "batch_max") { if (!(value >= 32 && value <= 4096) || value != std::floor(value)) FAIL(SNK_EINVAL, "batch_max must be an integer in 32..4096"); ctx->nmax = (int)value; }
   else if (k == "workspace_gb") { if (!(value > 0.0) || !std::isfinite(value)) FAIL(SNK_EINVAL, "workspace_gb must be > 0"); ctx->workspace_gb = value; }
+  else if (k == "tile_split") { if (!(value >= 0 && value <= 64) || value != std::floor(value)) FAIL(SNK_EINVAL, "tile_split must be an integer in 0..64 (0 = automatic)"); ctx->tile_split = (int)value; }
   else if (k == "atomics") { if (value != 1.0) FAIL(SNK_EINVAL, "atomics: only 1 is implemented"); }
   else FAIL(SNK_EINVAL, "unknown option key");
   ctx->have_grid = false;      // options take effect at the next snk_set_grid
@@ -775,11 +779,22 @@ static int build_impl(snk_ctx* ctx, const double* P, double* K, void* stream_, b
     ctx->n_launches += 1;
     ip.vlist = ctx->d_vlist.p; ip.vlstride = nunit; ip.vcnt = ctx->d_vcnt.p; ip.b0 = su.b0;
     ip.units = ctx->d_units.p; ip.meta = ctx->d_meta.p; ip.boys = ctx->d_boys.p;
-    // few tiles (large basis: the workspace holds few slots) would leave the last wave of a launch mostly empty: let several
-    // CTAs share a tile until there are some 4 000 CTAs (more than 8 waves of the 296-444 resident ones)
-    ip.nsplit = std::max(1, std::min(8, 4000 / std::max(1, ntiles)));
+    // CTAs per tile (each takes a contiguous share of the tile's unit list), chosen per class:
+    //  * L2: the CTAs of a launch that are resident at one time (about 3 per SM) re-read the F rows of their tiles once per
+    //    partner shell; with one tile per CTA those F blocks (nbf x 1 KB each) are hundreds of MB and the re-reads go to HBM.
+    //    Sharing a tile among n CTAs divides the resident blocks by n: n is set so that they fit about 48 MB of the 126 MB L2
+    //    (measured: config 3 build 1316 -> 1262 ms at n = 4..8, reduced-grid config 4 18.7 -> 16.8 s from n = 4 to 32);
+    //  * tail: a launch with few tiles (large basis, small super-batch) would leave its last wave mostly empty;
+    //  * but a CTA should keep about a thousand units of the class, else the per-CTA set-up shows (d-d: 60 % slower at n = 16).
+    auto split_for = [&](int c) {
+      if (ctx->tile_split > 0) return ctx->tile_split;
+      const int by_units = std::max(1, (ctx->cls_beg[c + 1] - ctx->cls_beg[c]) / 1024);
+      const int by_l2 = (int)std::ceil(3.0 * ctx->sm_count * (double)nbf * 1024.0 / 48e6);
+      const int by_tail = 4000 / std::max(1, ntiles);
+      return std::max(1, std::min(std::min(32, by_units), std::max(by_l2, by_tail)));
+    };
     for (int c = 0; c < kNumClasses; ++c) {
-      ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1]; ip.cls = c;
+      ip.pbeg = ctx->cls_beg[c]; ip.pend = ctx->cls_beg[c + 1]; ip.cls = c; ip.nsplit = split_for(c);
       if (ip.pend <= ip.pbeg) continue;
       auto spc = span_begin(ST_COUNT, c);
       CK(launch_integrals(c, ip, s));

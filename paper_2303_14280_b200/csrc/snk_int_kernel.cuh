@@ -293,17 +293,20 @@ __global__ void __launch_bounds__(int_threads(LA, LB), int_minblocks(LA, LB)) k_
   static_assert(NPM == 1 || NPM == 2 || NPM == 4, "points per thread");
   extern __shared__ __align__(128) unsigned char smem_int[];
 
-  // p.nsplit CTAs share a tile (launches with few tiles, e.g. a large basis on a small super-batch): CTA `part` takes every
-  // nsplit-th share of the unit list; G is accumulated with REDs anyway
+  // p.nsplit CTAs share a tile: CTA `part` takes the part-th contiguous range of the tile's unit list (contiguous, so that the
+  // runs of units with the same shell a stay together; G is accumulated with REDs anyway).  The CTAs of a tile have
+  // consecutive block indices, run at the same time and read the same F columns: fewer distinct tiles are resident, and the
+  // F block of a tile (nbf x 1 KB) is fetched from HBM once and shared through the L2.
   const int tile_id = blockIdx.x / p.nsplit, part = blockIdx.x - tile_id * p.nsplit;
   const TileRec tile = p.tiles[tile_id];
   const int jj = tile.batch - p.b0;
-  const int cnt = p.vcnt[jj * kNumClasses + p.cls];                  // units of this class kept by the tile's batch
+  const int cnt_all = p.vcnt[jj * kNumClasses + p.cls];              // units of this class kept by the tile's batch
+  const int lo = (int)((int64_t)cnt_all * part / p.nsplit), cnt = (int)((int64_t)cnt_all * (part + 1) / p.nsplit) - lo;
   if (cnt == 0) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int grp = warp / WPG, rnk = part * WPG + warp % WPG, stride = WPG * p.nsplit, pbase = grp * 32 * NPM;
+  const int grp = warp / WPG, rnk = warp % WPG, stride = WPG, pbase = grp * 32 * NPM;
   if (pbase >= tile.n) return;
-  const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg;
+  const int32_t* __restrict__ list = p.vlist + (int64_t)jj * p.vlstride + p.pbeg + lo;
   unsigned char* ring = smem_int + warp * (D * SLOT);
   const int need = min(NPM, (tile.n - pbase + 31) >> 5);   // point slots of the group that hold a point (ragged tiles)
   if (tile.n - pbase >= 32 * NPM) { consume_units<LA, LB, NPM, true>(p, tile, list, cnt, ring, pbase, rnk, stride, lane); return; }

@@ -47,7 +47,10 @@ static_assert(sizeof(UnitMeta) == 24, "UnitMeta layout");
 
 // A chunk = consecutive whole batches of one super-batch, up to kChunkSlots slots: the unit of the packed DMMA contractions
 // (snk_gemm_kt.cu).  Its row list (functions in the union of the batches' B_j) lives in a [nchunks x lstride] int table.
-constexpr int kChunkSlots = 2048;
+#ifndef SNK_CHUNK_SLOTS
+#define SNK_CHUNK_SLOTS 2048
+#endif
+constexpr int kChunkSlots = SNK_CHUNK_SLOTS;
 struct ChunkRec { int64_t slot0; int32_t nslots; int32_t b0, b1; int32_t pad; };
 static_assert(sizeof(ChunkRec) == 24, "ChunkRec layout");
 // 128-slot column tile of a4 (inside one chunk)
