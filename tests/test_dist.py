@@ -124,3 +124,20 @@ def test_world2_gloo_sharded_build_equals_single_build(oracle_mod):
     o.set_grid(w.points, w.weights, eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
     K1 = o.build_K(w.P)
     assert np.abs(K2 - K1).max() <= 1e-12 * max(1.0, np.abs(K1).max())
+
+
+def test_bench_oracle_sample_is_spatially_compact():
+    """bench.py sizes the timed oracle sample as a Morton-order prefix of whole root cells: a permutation whose prefixes are
+    compact boxes (so the oracle's octree makes batches of the usual size out of them), never scattered points."""
+    import bench
+    w = inputs.make_workload(2, grid=(10, 6, 12))
+    order = bench._morton_order(w.points, w.batch_cell)
+    assert np.array_equal(np.sort(order), np.arange(len(order)))
+    key = root_cell_keys(w.points[order], w.batch_cell)
+    assert len(np.unique(key)) == 1 + int(np.count_nonzero(np.diff(key)))           # every root cell is one contiguous run
+    # inside the most populated root cell a prefix is the lower octants (whole octree leaves), a strided sample spans the cell
+    uk, cnt = np.unique(key, return_counts=True)
+    cell = w.points[order][key == uk[np.argmax(cnt)]]            # Morton-ordered points of that cell
+    n = len(cell) // 16
+    vol = lambda p: float(np.prod(p.max(axis=0) - p.min(axis=0)))
+    assert vol(cell[:n]) < 0.5 * vol(cell[::16][:n])
