@@ -4,7 +4,7 @@
 //
 // B200 design (differs from the paper's A100 kernel):
 //   * the V_j bit masks are expanded once per super-batch into per-(batch, class) unit-id lists (k_vlist); the warps of a tile
-//     that cover the same points (a point group: the 8 warps for s-s, 4 of 8 for L = 1, 2 of 4 for L = 2, 3) take the list's
+//     that cover the same points (a point group: the 8 warps for s-s, the 4 warps for L = 1, 2 of 4 for L = 2, 3) take the list's
 //     entries round robin; when a launch has few tiles, several CTAs share a tile and split its list the same way;
 //   * every warp streams ITS units -- header + primitive pairs (<= 704 B) and the F_b row segments of its points -- through a
 //     private ring of D shared-memory slots with 16-byte cp.async copies, one commit group per unit: the warp refills a slot as
@@ -13,7 +13,7 @@
 //     allocated in warp pairs), no tickets, no barrier shared between warps.  (Bulk copies completing on mbarriers were
 //     measured first: one elected lane pays ~60 instructions per unit for the uniform-register set-up of 1 + ncart(l_b) copies;
 //     the per-lane 16-byte copies cost a fifth of that and need no barrier objects.);
-//   * a thread owns NP points of the tile (4 for s-s, 2 for L = 1..3, else 1): the point-independent work of a unit is paid
+//   * a thread owns NP points of the tile (4 for L <= 1, 2 for L = 2, 3, else 1): the point-independent work of a unit is paid
 //     once per 32 NP points and the NP recurrences are independent instruction streams;
 //   * the unit list is sorted by (a, b): G_a / F_a stay in registers over a run of units sharing a; G_b goes out with
 //     fire-and-forget RED.F64 (coalesced along the slot index);
@@ -34,7 +34,7 @@ namespace snk {
 #define SNK_NP_L0 4
 #endif
 #ifndef SNK_NP_L1
-#define SNK_NP_L1 2
+#define SNK_NP_L1 4
 #endif
 #ifndef SNK_NP_L2
 #define SNK_NP_L2 2
@@ -51,7 +51,7 @@ __host__ __device__ constexpr int int_npmax(int LA, int LB) {
 #define SNK_MB_L0 2
 #endif
 #ifndef SNK_MB_L1
-#define SNK_MB_L1 2
+#define SNK_MB_L1 3
 #endif
 #ifndef SNK_MB_L2
 #define SNK_MB_L2 3
@@ -72,7 +72,7 @@ __host__ __device__ constexpr int int_minblocks(int LA, int LB) {
 #define SNK_CW_L0 8
 #endif
 #ifndef SNK_CW_L1
-#define SNK_CW_L1 8
+#define SNK_CW_L1 4
 #endif
 #ifndef SNK_CW_L2
 #define SNK_CW_L2 4
