@@ -10,10 +10,13 @@ a0/a1 are per-geometry and reported as ``set_grid_ms``) over the synthetic workl
 ``e2e``    = the same through ``snk_build_K_host`` (HOST P in, HOST K out; H2D/D2H inside the timed region).
 ``roofline``: dominant integral-contraction kernel (bound "alu": plain FP64 DFMA pipe) -- algorithmic flops of its
 launch (DESIGN.md flop model) / its CUDA-event duration inside the timed region / measured DFMA peak of this GPU.
-``cpu_baseline``: the oracle, as it stands, on the host cores, on a bounded sample (whole root cells, R13).
+``cpu_baseline``: the oracle, as it stands, on the host cores, on a bounded, spatially compact sample (whole root cells of
+R13 when the budget covers them, else a Morton-order prefix of the first ones); ``--impl reference`` times that same sample.
 
-N > 1 (torchrun): the grid's root cells are dealt to ranks by Alg. 2 (greedy LPT), every rank
-builds its partial K and one NCCL all-reduce (Alg. 1 line 13) sums them -- strong scaling of one build.
+N > 1 (torchrun): by default every rank builds K for its own density on the whole grid (independent problems, no collective:
+weak scaling).  ``--multi shard``: one screening pass gives the primitive pair-points of every batch, root cells are dealt to
+ranks by Alg. 2 on them (greedy LPT), every rank builds its partial K and one NCCL all-reduce (Alg. 1 line
+13) sums them -- strong scaling of one build.
 """
 from __future__ import annotations
 
