@@ -148,44 +148,54 @@ def time_oracle_sample(w, target_s=15.0, first_frac=0.01, return_idx=False):
                 seconds=dt, n_int=st["n_int_contracted"])
 
 
-def run_reference(args, rank, world):
-    """--impl reference: the oracle on the host cores, same config/metric.  The sample is sized ONCE exactly as the
-    `cpu_baseline` leg of the GPU arm sizes it (whole root cells in R13 hash order, about --cpu-seconds of host time, no
-    thinning unless one root cell is already too much) and every step times the oracle's K build on that same sample, so the
-    rate is the cpu_baseline's rate; the grid is generated on the same device as in the GPU arm (same points and weights)."""
-    if rank != 0:
-        return
-    from oracle import oracle as orc
-    from paper_2303_14280_b200 import inputs
-    w = inputs.make_workload(args.config, grid=args.grid, device=_gen_device(), density=args.density)
-    # per-step budget: the whole --steps K --warmup W run has to end within minutes (about 1000 s of oracle time at most)
+def oracle_sample_for(w, args):
+    """The ONE oracle sample both arms time (the driver passes the same --steps / --warmup to both): sized for a per-step
+    budget such that the reference arm's whole run ends within minutes (about 1000 s of oracle time at most), cut back along
+    the Morton curve when the sizing pass overshot it.  Returns (point indices, how it was chosen)."""
     budget = min(args.cpu_seconds, 1000.0 / (args.steps + args.warmup + 3))
     first = time_oracle_sample(w, target_s=budget, return_idx=True)
     idx = first.pop("idx")
     if first["seconds"] > 1.25 * budget and first["sample"].startswith("spatially"):
         # the cost per point grows along the Morton curve (towards the nuclei): cut the prefix back to the budget
         idx = idx[:max(256, int(len(idx) * budget / first["seconds"]))]
+    return idx, first["sample"].split(":")[0]
+
+
+def time_oracle_on(w, idx, how, nrep=1, nwarm=0):
+    """The oracle's K build on the points idx, nwarm untimed + nrep timed builds -> (rate, seconds per build, cores, sample line)."""
+    from oracle import oracle as orc
     o = orc.Oracle(w.basis)
     o.set_grid(w.points[idx], w.weights[idx], eps=w.eps, batch_cell=w.batch_cell, batch_max=w.batch_max)
     res = []
-    for i in range(args.warmup + args.steps):
+    for i in range(nwarm + nrep):
         t = time.time()
         o.build_K(w.P)
         dt = time.time() - t
-        if i >= args.warmup:
+        if i >= nwarm:
             res.append(dt)
     st = o.stats()
     n_int = st["n_int_contracted"]
-    secs = sum(res)
-    val = n_int * len(res) / secs
     nb = len(o.batches()[0]) - 1
     used = int(min(st["threads"], max(nb, 1)))
     npts = w.points.shape[0]
     sample = ("%s: %d of %d points (%.3f%%) in %d batches on %d OpenMP threads (parallel over batches: %d had work), %.3g contracted "
-              "integrals per step; oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned"
-              % (first["sample"].split(":")[0], len(idx), npts, 100.0 * len(idx) / npts, nb, st["threads"], used, n_int))
+              "integrals per build, %.1f s per build; oracle = C++ -O2 -fopenmp McMurchie-Davidson, untuned"
+              % (how, len(idx), npts, 100.0 * len(idx) / npts, nb, st["threads"], used, n_int, sum(res) / len(res)))
+    return n_int * len(res) / sum(res), sum(res) / len(res), used, sample
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, same config/metric.  Both arms call oracle_sample_for with the same
+    flags, so the sample timed here step by step is the one the GPU arm's `cpu_baseline` leg times once; the grid is generated
+    on the same device as in the GPU arm (same points and weights)."""
+    if rank != 0:
+        return
+    from paper_2303_14280_b200 import inputs
+    w = inputs.make_workload(args.config, grid=args.grid, device=_gen_device(), density=args.density)
+    idx, how = oracle_sample_for(w, args)
+    val, per_build, used, sample = time_oracle_on(w, idx, how, nrep=args.steps, nwarm=args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, len(res)), "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": 1e3 * per_build, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": _workload_name(args.config, w), "sample": sample, "density": args.density, "batch_cell": w.batch_cell, "batch_max": w.batch_max},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
@@ -411,8 +421,9 @@ def main():
                       "nsuper": st["nsuper"], "fp64_peak_tflops": {"dfma": dfma_peak, "dmma": dmma_peak},
                       "whole_build_fp64_frac": (st["flops_integral"] + st["flops_gemm"]) / (st["ms_build"] * 1e-3) * 1e-12 / dfma_peak}}
     if not args.no_cpu_baseline:
-        cb = time_oracle_sample(w, target_s=args.cpu_seconds)
-        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        idx, how = oracle_sample_for(w, args)                  # the sample `--impl reference` times with the same flags
+        val, _, used, sample = time_oracle_on(w, idx, how, nrep=1, nwarm=1)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
